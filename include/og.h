@@ -1,0 +1,197 @@
+/*
+ * og.h -- C ABI of libogtree.so: B200-native TreePM short-range gravity
+ *         (tree construction + Barnes-Hut tree walk), single GPU, sm_100a.
+ *
+ * What the calls compute.  The paper states the problem only qualitatively: "for each
+ * dynamically active particle, a tree walk is performed to compute the forces acting on
+ * it" (Sec. 2), Barnes & Hut gravity opened by a criterion,
+ * TreePM with the long-range part done elsewhere.  It prints no formula;
+ * the arithmetic is the reading fixed in SURVEY.md Sec. 8.3 (C0..C7, R1..R30) and listed
+ * in DESIGN.md Sec. 3.  Each entry point below cites the item it implements.
+ *
+ * Conventions (all entry points)
+ *  - Every pointer says DEVICE or HOST.  Device pointers must be valid on the current
+ *    CUDA device; inputs are borrowed and only read; outputs are caller-owned.
+ *  - `stream` is a cudaStream_t passed as an opaque pointer (NULL = legacy default
+ *    stream).  Calls only ENQUEUE work on `stream` and return; the library never calls
+ *    cudaDeviceSynchronize.  Inputs must stay valid until the stream has passed the call.
+ *  - `int` functions return OG_OK (0) or a negative og_status; og_tree_build returns NULL
+ *    on synchronous failure.  og_last_error() holds a thread-local message for the last
+ *    failing call.  No C++ exception crosses the ABI; nothing aborts.
+ *  - Conditions detected on the device (node capacity exceeded, walk stack overflow,
+ *    position outside [0, box) when OG_VALIDATE_POS) are latched in the tree and returned
+ *    by og_tree_status().
+ *  - There is no CPU fallback: without a CUDA device every compute call fails with
+ *    OG_ERR_CUDA.
+ */
+#ifndef OG_H
+#define OG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct og_tree og_tree;         /* opaque; device-resident; owned by the library */
+typedef struct CUstream_st *og_stream;  /* == cudaStream_t */
+
+typedef enum {
+    OG_OK = 0,
+    OG_ERR_INVALID_ARG = -1,
+    OG_ERR_OUT_OF_MEMORY = -2,
+    OG_ERR_NODE_OVERFLOW = -3,   /* canonical octree needs more than max_nodes nodes (R6)  */
+    OG_ERR_CUDA = -4,
+    OG_ERR_BAD_POSITION = -5,    /* OG_VALIDATE_POS: some x not in [0, box)                */
+    OG_ERR_STACK_OVERFLOW = -6   /* walk traversal stack exceeded its spill capacity       */
+} og_status;
+
+/* og_params.flags */
+#define OG_PERIODIC 1u      /* required in this build (nearest-image distances, R13)      */
+#define OG_VALIDATE_POS 2u  /* device-side check 0 <= x < box during key generation       */
+#define OG_COUNT 4u         /* walk also accumulates interaction counters (og_stats)      */
+
+/* og_params.walk_variant */
+#define OG_WALK_DEFAULT 0u  /* warp-cooperative group walk (the product path)             */
+#define OG_WALK_SIMPLE 1u   /* one thread per target, private stack (debug / comparison)  */
+
+typedef struct {
+    uint32_t struct_size;   /* = sizeof(og_params); ABI guard                              */
+    uint32_t flags;         /* OG_PERIODIC | ...                                           */
+    float G;                /* gravitational constant (R12; 1 in all configs)              */
+    float r_s;              /* force-split scale, same units as box                        */
+    float rcut_over_rs;     /* 4.5 (BASELINE.json north_star)                              */
+    float alpha;            /* relative opening criterion (R14), used iff a_old != NULL    */
+    float theta;            /* geometric criterion (R22), used iff a_old == NULL           */
+    uint32_t leaf_max;      /* bucket size of the canonical octree (R7), default 8         */
+    uint32_t max_nodes;     /* node capacity; 0 -> default (R6)                            */
+    uint32_t walk_variant;  /* OG_WALK_*                                                   */
+    void *workspace;        /* DEVICE scratch supplied by the caller, or NULL -> the       */
+    size_t workspace_bytes; /* library allocates with cudaMallocAsync on `stream`          */
+} og_params;
+
+typedef struct {
+    uint64_t n;             /* particles                                                   */
+    uint64_t n_nodes;       /* nodes of the canonical octree                               */
+    uint32_t max_level;     /* deepest level holding a node (root = 0)                     */
+    uint32_t reserved;
+    /* sums over the targets of the last og_shortrange_accel with OG_COUNT (else 0):       */
+    uint64_t V_full;        /* visits that passed the cull                                 */
+    uint64_t V_cull;        /* visits removed by the cutoff-box test                       */
+    uint64_t A_in;          /* accepted nodes with r < r_cut                               */
+    uint64_t P_in;          /* particle pairs with r < r_cut                               */
+    uint64_t P_soft;        /* ... of which r < h                                          */
+    uint64_t P_out;         /* particle pairs evaluated with r >= r_cut                    */
+    uint64_t fp64_rechecks; /* decisions re-evaluated in fp64           */
+} og_stats;
+
+/* og_tree_get field selectors.  Pointers are DEVICE pointers into the tree, valid until
+ * og_tree_free; `count` is the number of ELEMENTS of the stated type.                    */
+typedef enum {
+    OG_F_KEYS_SORTED = 0,   /* u64 [n]     Morton keys in sorted order (C1, C2)            */
+    OG_F_PERM = 1,          /* u32 [n]     perm[s] = original index of sorted slot s (C2)  */
+    OG_F_INV_PERM = 2,      /* u32 [n]     inverse permutation                             */
+    OG_F_SPOS = 3,          /* f32 [n][4]  sorted (x, y, z, m)                             */
+    OG_F_SH = 4,            /* f32 [n]     sorted h = fl32(2.8 eps) (R9)                   */
+    OG_F_NODE_LEVEL = 5,    /* u8  [n_nodes]                                               */
+    OG_F_NODE_FIRST = 6,    /* u32 [n_nodes] first sorted slot                             */
+    OG_F_NODE_COUNT = 7,    /* u32 [n_nodes] particle count                                */
+    OG_F_NODE_FIRST_CHILD = 8, /* u32 [n_nodes] (0 for leaves)                             */
+    OG_F_NODE_NCHILD = 9,   /* u8  [n_nodes] 0 for leaves, else 1..8                       */
+    OG_F_NODE_COM = 10,     /* f32 [n_nodes][4]  (s_x, s_y, s_z, M)        fp32 record R9  */
+    OG_F_NODE_CELL = 11,    /* f32 [n_nodes][4]  (c_x, c_y, c_z, l)                        */
+    OG_F_NODE_LO = 12,      /* f32 [n_nodes][4]  (lo_x, lo_y, lo_z, h_max)  tight AABB     */
+    OG_F_NODE_HI = 13,      /* f32 [n_nodes][4]  (hi_x, hi_y, hi_z, unused)                */
+    OG_F_LEVEL_START = 14   /* u32 [23]    node index where each level starts (BFS)        */
+} og_field;
+
+/* Bytes of DEVICE workspace og_tree_build needs for n particles (0 on invalid input).    */
+size_t og_tree_workspace_bytes(uint64_t n, const og_params *params);
+
+/*
+ * Rows a1..a5 of SURVEY.md Sec. 8: Morton keys (C1) -> stable LSD radix sort with index
+ * tie-break (C2) -> gather to sorted float4 (x,y,z,m) + h -> canonical sparse octree (C3)
+ * -> upward pass (C4: M, centre of mass, cell centre/side, tight AABB, h_max; fp64
+ * accumulation in slot / child order, stored fp32).
+ *   pos   DEVICE f32 [n][3], 0 <= x < box       (borrowed)
+ *   mass  DEVICE f32 [n]                        (borrowed)
+ *   soft  DEVICE f32 [n]  Plummer-equivalent eps; h = 2.8 eps (borrowed)
+ *   n     1 <= n < 2^31;   box > 0;   requires rcut_over_rs * r_s < box / 2 (R13)
+ * Returns a tree that owns sorted copies (inputs may be released once the stream has
+ * passed the call), or NULL (bad struct_size / sizes / pointers, r_cut >= box/2,
+ * leaf_max == 0, allocation failure).  Cite: PAPER.md:88, :322 (the reference builds its
+ * tree on the CPU and re-uploads it; here it is built on the device).
+ */
+og_tree *og_tree_build(const float *pos, const float *mass, const float *soft, uint64_t n,
+                       float box, const og_params *params, og_stream stream);
+
+/*
+ * Rows a6..a7: short-range tree walk (C5, C6) for the active targets and scatter of the
+ * results in the caller's order.  PAPER.md:59 ("for each dynamically active particle a
+ * tree walk"), :74 (per-node interaction, opening criterion).
+ *   active_idx DEVICE u32 [n_active] ORIGINAL particle indices, any order, no duplicates
+ *              required; NULL -> all n particles in identity order (n_active must be n)
+ *   a_old      DEVICE f32 [n_active] |a| of the previous step in active order (R23);
+ *              NULL -> geometric criterion l^2 > theta^2 r^2 (R22)
+ *   acc_out    DEVICE f32 [n_active][3], overwritten
+ *   pot_out    DEVICE f32 [n_active], overwritten, or NULL
+ * Returns OG_OK or a negative og_status (also a previously latched device condition).
+ */
+int og_shortrange_accel(const og_tree *tree, const uint32_t *active_idx, uint64_t n_active,
+                        const float *a_old, float *acc_out, float *pot_out, og_stream stream);
+
+/* DEVICE pointer + element count of one tree array (og_field).  Synchronises the tree's
+ * build stream once (to learn n_nodes).                                                   */
+int og_tree_get(const og_tree *tree, int field, const void **dev_ptr, uint64_t *count);
+
+/* Synchronises the stream(s) the tree was used on; returns the latched status.           */
+int og_tree_status(const og_tree *tree);
+
+/* Synchronises like og_tree_status and fills *stats.                                     */
+int og_tree_stats(const og_tree *tree, og_stats *stats);
+
+/* Releases the tree (stream-ordered on `stream`).  NULL is ignored.                      */
+void og_tree_free(og_tree *tree, og_stream stream);
+
+/* Thread-local message of the last failing call ("" if none).                            */
+const char *og_last_error(void);
+
+/* ---- single rows, exposed for parity tests and per-kernel measurement ---------------- */
+
+/* Row a1 (C1, R1, R2): key[i] = Morton(quantise(pos[i])), idx[i] = i.
+ *   pos DEVICE f32 [n][3];  keys DEVICE u64 [n];  idx DEVICE u32 [n] or NULL.            */
+int og_morton_keys(const float *pos, uint64_t n, float box, uint64_t *keys, uint32_t *idx,
+                   og_stream stream);
+
+/* Bytes of DEVICE scratch og_radix_sort_pairs needs for n pairs.                          */
+size_t og_radix_sort_scratch_bytes(uint64_t n);
+
+/* Row a2 (C2, R3): stable LSD radix sort of (key, val) pairs by key bits
+ * [begin_bit, end_bit), 8 bits per pass.  keys/vals are DEVICE ping-pong buffers of n
+ * elements each; on return *result_in_alt = 1 if the sorted data is in (keys_alt,
+ * vals_alt), else 0 (it is in keys/vals).  Stability gives the index tie-break.           */
+int og_radix_sort_pairs(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint32_t *vals_alt,
+                        uint64_t n, int begin_bit, int end_bit, void *scratch,
+                        size_t scratch_bytes, int *result_in_alt, og_stream stream);
+
+/*
+ * End-to-end convenience with HOST buffers (bench.py's `e2e` leg): copies pos/mass/soft
+ * (and active_idx, a_old if given) to the device, runs og_tree_build + og_shortrange_accel,
+ * copies acc/pot back, frees everything, and synchronises `stream` before returning.
+ * All pointers HOST (pinned memory recommended); semantics as the two calls above.
+ */
+int og_shortrange_accel_host(const float *pos, const float *mass, const float *soft, uint64_t n,
+                             float box, const og_params *params, const uint32_t *active_idx,
+                             uint64_t n_active, const float *a_old, float *acc_out,
+                             float *pot_out, og_stream stream);
+
+/* FP32 FFMA micro-benchmark used by bench.py to state the measured ALU peak next to the
+ * nominal one: runs `iters` dependent-chain FFMAs x 8 chains per thread on every SM and
+ * returns the elapsed milliseconds (CUDA events, synchronises) and the flop count.        */
+int og_ffma_peak_probe(uint64_t iters, double *ms_out, double *flops_out, og_stream stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OG_H */

@@ -1,0 +1,429 @@
+// api.cu -- the C ABI of include/og.h: argument checks, device arena layout, stream-ordered
+// launch sequences.  Every step of the path runs in the kernels of this directory; there is no
+// CPU fallback.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "og_internal.cuh"
+
+static thread_local char g_err[512] = "";
+
+void og_set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+extern "C" const char *og_last_error(void) { return g_err; }
+
+namespace {
+
+inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Layout {
+    size_t keysA, keysB, idxA, idxB, sort_scratch, spos, sh, inv_perm;
+    size_t level, first, count, first_child, nchild, com, cell, lo, hi, info;
+    size_t oct_scratch, level_start, status, counters, split_tab, spill, total;
+};
+
+Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count)
+{
+    Layout L;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
+    L.keysA = take(n * 8); L.keysB = take(n * 8);
+    L.idxA = take(n * 4);  L.idxB = take(n * 4);
+    L.sort_scratch = take(ogk_sort_scratch_bytes(n));
+    L.spos = take(n * 16); L.sh = take(n * 4); L.inv_perm = take(n * 4);
+    const size_t M = max_nodes;
+    L.level = take(M); L.first = take(M * 4); L.count = take(M * 4); L.first_child = take(M * 4);
+    L.nchild = take(M);
+    L.com = take(M * 16); L.cell = take(M * 16); L.lo = take(M * 16); L.hi = take(M * 16);
+    L.info = take(M * 8);
+    L.oct_scratch = take(ogk_octree_scratch_bytes(max_nodes));
+    L.level_start = take(24 * 4);
+    L.status = take(16 * 4);
+    L.counters = take(OGC_N * 8);
+    L.split_tab = take(1024 * 16);
+    L.spill = take(ogk_walk_spill_bytes(sm_count));
+    L.total = o;
+    return L;
+}
+
+uint32_t default_max_nodes(uint64_t n, const og_params *p)
+{
+    if (p->max_nodes) return p->max_nodes;
+    // R6: observed nodes/N is 0.14..0.49 at leaf_max = 8 and 1.49 at leaf_max = 1
+    uint64_t m = (p->leaf_max >= 4) ? n : 3 * n;
+    if (m < 4096) m = 4096;
+    if (m > 0x7fffffffull) m = 0x7fffffffull;
+    return (uint32_t)m;
+}
+
+bool check_params(const og_params *p, uint64_t n, float box)
+{
+    if (!p) { og_set_error("params is NULL"); return false; }
+    if (p->struct_size != sizeof(og_params)) {
+        og_set_error("og_params.struct_size = %u, expected %zu", p->struct_size, sizeof(og_params));
+        return false;
+    }
+    if (n == 0 || n >= (1ull << 31)) { og_set_error("n = %llu out of range [1, 2^31)", (unsigned long long)n); return false; }
+    if (!(box > 0.0f)) { og_set_error("box must be > 0"); return false; }
+    if (!(p->flags & OG_PERIODIC)) { og_set_error("OG_PERIODIC is required in this build"); return false; }
+    if (p->leaf_max == 0) { og_set_error("leaf_max must be >= 1"); return false; }
+    if (!(p->r_s > 0.0f) || !(p->rcut_over_rs > 0.0f)) { og_set_error("r_s and rcut_over_rs must be > 0"); return false; }
+    if (!((double)p->rcut_over_rs * (double)p->r_s < 0.5 * (double)box)) {
+        og_set_error("r_cut = %g must be < box/2 = %g (nearest-image convention, R13)",
+                     (double)p->rcut_over_rs * (double)p->r_s, 0.5 * (double)box);
+        return false;
+    }
+    if (p->walk_variant > OG_WALK_SIMPLE) { og_set_error("unknown walk_variant %u", p->walk_variant); return false; }
+    return true;
+}
+
+int device_sm_count(int *device_out)
+{
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
+    if (device_out) *device_out = dev;
+    return sms;
+}
+
+int status_from_bits(uint32_t bits)
+{
+    if (bits & OG_DEV_NODE_OVERFLOW) return OG_ERR_NODE_OVERFLOW;
+    if (bits & OG_DEV_BAD_POSITION) return OG_ERR_BAD_POSITION;
+    if (bits & OG_DEV_STACK_OVERFLOW) return OG_ERR_STACK_OVERFLOW;
+    if (bits & OG_DEV_BAD_INDEX) return OG_ERR_INVALID_ARG;
+    return OG_OK;
+}
+
+// Synchronises the streams the tree has been used on and refreshes the host copies.
+int tree_sync(const og_tree *t, uint32_t *bits_out)
+{
+    OG_CUDA_TRY(cudaStreamSynchronize(t->build_stream), return OG_ERR_CUDA);
+    if (t->last_stream != t->build_stream) OG_CUDA_TRY(cudaStreamSynchronize(t->last_stream), return OG_ERR_CUDA);
+    uint32_t ls[24];
+    OG_CUDA_TRY(cudaMemcpy(ls, t->d_level_start, sizeof(ls), cudaMemcpyDeviceToHost), return OG_ERR_CUDA);
+    t->n_nodes_host = ls[22];
+    uint32_t ml = 0;
+    for (uint32_t lv = 0; lv <= OG_MAX_LEVEL; ++lv)
+        if (ls[lv + 1] > ls[lv]) ml = lv;
+    t->max_level_host = ml;
+    uint32_t bits = 0;
+    OG_CUDA_TRY(cudaMemcpy(&bits, t->d_status, sizeof(bits), cudaMemcpyDeviceToHost), return OG_ERR_CUDA);
+    if (bits_out) *bits_out = bits;
+    return OG_OK;
+}
+
+}  // namespace
+
+extern "C" size_t og_tree_workspace_bytes(uint64_t n, const og_params *params)
+{
+    if (!params || params->struct_size != sizeof(og_params) || n == 0 || n >= (1ull << 31)) return 0;
+    int sms = device_sm_count(nullptr);
+    if (sms <= 0) sms = 148;  // no device visible: size for a B200
+    return make_layout(n, default_max_nodes(n, params), sms).total;
+}
+
+extern "C" og_tree *og_tree_build(const float *pos, const float *mass, const float *soft, uint64_t n,
+                                  float box, const og_params *params, og_stream stream)
+{
+    g_err[0] = 0;
+    if (!check_params(params, n, box)) return nullptr;
+    if (!pos || !mass || !soft) { og_set_error("pos / mass / soft must be non-NULL device pointers"); return nullptr; }
+    int dev = 0;
+    const int sms = device_sm_count(&dev);
+    if (sms <= 0) { og_set_error("no CUDA device available (there is no CPU fallback)"); return nullptr; }
+    cudaStream_t st = (cudaStream_t)stream;
+    og_tree *t = new (std::nothrow) og_tree();
+    if (!t) { og_set_error("host allocation failed"); return nullptr; }
+    memset(t, 0, sizeof(*t));
+    t->n = n; t->box = box; t->prm = *params; t->device = dev; t->sm_count = sms;
+    t->max_nodes = default_max_nodes(n, params);
+    t->build_stream = st; t->last_stream = st; t->n_nodes_host = -1;
+    const Layout L = make_layout(n, t->max_nodes, sms);
+    if (params->workspace) {
+        if (params->workspace_bytes < L.total || ((uintptr_t)params->workspace & 255u)) {
+            og_set_error("workspace too small or not 256-byte aligned: %zu bytes given, %zu needed",
+                         params->workspace_bytes, L.total);
+            delete t;
+            return nullptr;
+        }
+        t->arena = params->workspace; t->owns_arena = 0;
+    } else {
+        cudaError_t e = cudaMallocAsync(&t->arena, L.total, st);
+        if (e != cudaSuccess) {
+            og_set_error("cudaMallocAsync(%zu bytes) failed: %s", L.total, cudaGetErrorString(e));
+            (void)cudaGetLastError();
+            delete t;
+            return nullptr;
+        }
+        t->owns_arena = 1;
+    }
+    t->arena_bytes = L.total;
+    char *b = reinterpret_cast<char *>(t->arena);
+    uint64_t *keysA = (uint64_t *)(b + L.keysA), *keysB = (uint64_t *)(b + L.keysB);
+    uint32_t *idxA = (uint32_t *)(b + L.idxA), *idxB = (uint32_t *)(b + L.idxB);
+    t->spos = (float4 *)(b + L.spos); t->sh = (float *)(b + L.sh); t->inv_perm = (uint32_t *)(b + L.inv_perm);
+    t->node_level = (uint8_t *)(b + L.level); t->node_first = (uint32_t *)(b + L.first);
+    t->node_count = (uint32_t *)(b + L.count); t->node_first_child = (uint32_t *)(b + L.first_child);
+    t->node_nchild = (uint8_t *)(b + L.nchild);
+    t->node_com = (float4 *)(b + L.com); t->node_cell = (float4 *)(b + L.cell);
+    t->node_lo = (float4 *)(b + L.lo); t->node_hi = (float4 *)(b + L.hi); t->node_info = (uint2 *)(b + L.info);
+    t->d_level_start = (uint32_t *)(b + L.level_start); t->d_status = (uint32_t *)(b + L.status);
+    t->d_counters = (unsigned long long *)(b + L.counters);
+    t->split_tab = (float4 *)(b + L.split_tab);
+    t->walk_spill = b + L.spill; t->walk_spill_bytes = ogk_walk_spill_bytes(sms);
+
+#define OG_BUILD_TRY(expr)                                                    \
+    OG_CUDA_TRY(expr, {                                                       \
+        if (t->owns_arena) cudaFreeAsync(t->arena, st);                       \
+        delete t;                                                             \
+        return nullptr;                                                       \
+    })
+    // level_start, status, counters are adjacent: clear them in one memset
+    OG_BUILD_TRY(cudaMemsetAsync(b + L.level_start, 0, L.split_tab - L.level_start, st));
+    OG_BUILD_TRY(ogk_keys(pos, n, box, keysA, idxA, t->d_status, (params->flags & OG_VALIDATE_POS) != 0, st));
+    int in_alt = 0;
+    OG_BUILD_TRY(ogk_radix_sort(keysA, idxA, keysB, idxB, n, 0, 64, b + L.sort_scratch, &in_alt, st));
+    t->keys = in_alt ? keysB : keysA;
+    t->perm = in_alt ? idxB : idxA;
+    OG_BUILD_TRY(ogk_gather(pos, mass, soft, t->perm, n, t->spos, t->sh, t->inv_perm, st));
+    OG_BUILD_TRY(ogk_split_table(t->split_tab, (double)params->rcut_over_rs * (double)params->r_s,
+                                 (double)params->r_s, st));
+    OG_BUILD_TRY(ogk_octree_upward(t, b + L.oct_scratch, st));
+#undef OG_BUILD_TRY
+    return t;
+}
+
+extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx, uint64_t n_active,
+                                   const float *a_old, float *acc_out, float *pot_out, og_stream stream)
+{
+    g_err[0] = 0;
+    if (!t) { og_set_error("tree is NULL"); return OG_ERR_INVALID_ARG; }
+    if (!acc_out) { og_set_error("acc_out is NULL"); return OG_ERR_INVALID_ARG; }
+    if (!active_idx && n_active != t->n) {
+        og_set_error("active_idx == NULL requires n_active == n (%llu != %llu)", (unsigned long long)n_active,
+                     (unsigned long long)t->n);
+        return OG_ERR_INVALID_ARG;
+    }
+    if (n_active >= (1ull << 31)) { og_set_error("n_active out of range"); return OG_ERR_INVALID_ARG; }
+    if (n_active == 0) return OG_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    t->last_stream = st;
+    if (!active_idx) {
+        OG_CUDA_TRY(ogk_walk(t, nullptr, t->perm, n_active, a_old, acc_out, pot_out, st), return OG_ERR_CUDA);
+        return OG_OK;
+    }
+    // active subset: order the targets by sorted slot so that a warp's 32 targets are neighbours
+    const size_t na = (size_t)n_active;
+    const size_t o_k0 = 0, o_k1 = align_up(na * 8), o_v0 = o_k1 + align_up(na * 8), o_v1 = o_v0 + align_up(na * 4),
+                 o_sl = o_v1 + align_up(na * 4), o_sc = o_sl + align_up(na * 4),
+                 total = o_sc + align_up(ogk_sort_scratch_bytes(n_active));
+    char *tmp = nullptr;
+    cudaError_t e = cudaMallocAsync((void **)&tmp, total, st);
+    if (e != cudaSuccess) {
+        og_set_error("cudaMallocAsync(%zu bytes) failed: %s", total, cudaGetErrorString(e));
+        (void)cudaGetLastError();
+        return OG_ERR_OUT_OF_MEMORY;
+    }
+    uint64_t *k0 = (uint64_t *)(tmp + o_k0), *k1 = (uint64_t *)(tmp + o_k1);
+    uint32_t *v0 = (uint32_t *)(tmp + o_v0), *v1 = (uint32_t *)(tmp + o_v1), *slots = (uint32_t *)(tmp + o_sl);
+    int bits = 1;
+    while (bits < 32 && (1ull << bits) < t->n) ++bits;
+    int in_alt = 0;
+#define OG_ACC_TRY(expr) OG_CUDA_TRY(expr, { cudaFreeAsync(tmp, st); return OG_ERR_CUDA; })
+    OG_ACC_TRY(ogk_active_slots(active_idx, t->inv_perm, t->n, n_active, k0, v0, t->d_status, st));
+    OG_ACC_TRY(ogk_radix_sort(k0, v0, k1, v1, n_active, 0, bits, tmp + o_sc, &in_alt, st));
+    OG_ACC_TRY(ogk_unpack_slots(in_alt ? k1 : k0, n_active, slots, st));
+    OG_ACC_TRY(ogk_walk(t, slots, in_alt ? v1 : v0, n_active, a_old, acc_out, pot_out, st));
+    OG_ACC_TRY(cudaFreeAsync(tmp, st));
+#undef OG_ACC_TRY
+    return OG_OK;
+}
+
+extern "C" int og_tree_get(const og_tree *t, int field, const void **dev_ptr, uint64_t *count)
+{
+    g_err[0] = 0;
+    if (!t || !dev_ptr || !count) { og_set_error("NULL argument"); return OG_ERR_INVALID_ARG; }
+    if (t->n_nodes_host < 0) {
+        const int rc = tree_sync(t, nullptr);
+        if (rc != OG_OK) return rc;
+    }
+    const uint64_t nn = (uint64_t)t->n_nodes_host;
+    switch (field) {
+    case OG_F_KEYS_SORTED: *dev_ptr = t->keys; *count = t->n; break;
+    case OG_F_PERM: *dev_ptr = t->perm; *count = t->n; break;
+    case OG_F_INV_PERM: *dev_ptr = t->inv_perm; *count = t->n; break;
+    case OG_F_SPOS: *dev_ptr = t->spos; *count = t->n * 4; break;
+    case OG_F_SH: *dev_ptr = t->sh; *count = t->n; break;
+    case OG_F_NODE_LEVEL: *dev_ptr = t->node_level; *count = nn; break;
+    case OG_F_NODE_FIRST: *dev_ptr = t->node_first; *count = nn; break;
+    case OG_F_NODE_COUNT: *dev_ptr = t->node_count; *count = nn; break;
+    case OG_F_NODE_FIRST_CHILD: *dev_ptr = t->node_first_child; *count = nn; break;
+    case OG_F_NODE_NCHILD: *dev_ptr = t->node_nchild; *count = nn; break;
+    case OG_F_NODE_COM: *dev_ptr = t->node_com; *count = nn * 4; break;
+    case OG_F_NODE_CELL: *dev_ptr = t->node_cell; *count = nn * 4; break;
+    case OG_F_NODE_LO: *dev_ptr = t->node_lo; *count = nn * 4; break;
+    case OG_F_NODE_HI: *dev_ptr = t->node_hi; *count = nn * 4; break;
+    case OG_F_LEVEL_START: *dev_ptr = t->d_level_start; *count = 23; break;
+    default: og_set_error("unknown field %d", field); return OG_ERR_INVALID_ARG;
+    }
+    return OG_OK;
+}
+
+extern "C" int og_tree_status(const og_tree *t)
+{
+    g_err[0] = 0;
+    if (!t) { og_set_error("tree is NULL"); return OG_ERR_INVALID_ARG; }
+    uint32_t bits = 0;
+    const int rc = tree_sync(t, &bits);
+    if (rc != OG_OK) return rc;
+    const int s = status_from_bits(bits);
+    if (s != OG_OK) og_set_error("device-latched status bits 0x%x", bits);
+    return s;
+}
+
+extern "C" int og_tree_stats(const og_tree *t, og_stats *out)
+{
+    g_err[0] = 0;
+    if (!t || !out) { og_set_error("NULL argument"); return OG_ERR_INVALID_ARG; }
+    const int rc = tree_sync(t, nullptr);
+    if (rc != OG_OK) return rc;
+    unsigned long long c[OGC_N];
+    OG_CUDA_TRY(cudaMemcpy(c, t->d_counters, sizeof(c), cudaMemcpyDeviceToHost), return OG_ERR_CUDA);
+    memset(out, 0, sizeof(*out));
+    out->n = t->n; out->n_nodes = (uint64_t)t->n_nodes_host; out->max_level = t->max_level_host;
+    out->V_full = c[OGC_V_FULL]; out->V_cull = c[OGC_V_CULL]; out->A_in = c[OGC_A_IN];
+    out->P_in = c[OGC_P_IN]; out->P_soft = c[OGC_P_SOFT]; out->P_out = c[OGC_P_OUT];
+    out->fp64_rechecks = c[OGC_FP64];
+    return OG_OK;
+}
+
+extern "C" void og_tree_free(og_tree *t, og_stream stream)
+{
+    if (!t) return;
+    if (t->owns_arena && t->arena) {
+        // the arena may still be in use on another stream: order the free after it
+        if (t->last_stream != (cudaStream_t)stream) cudaStreamSynchronize(t->last_stream);
+        cudaFreeAsync(t->arena, (cudaStream_t)stream);
+    }
+    delete t;
+}
+
+extern "C" int og_morton_keys(const float *pos, uint64_t n, float box, uint64_t *keys, uint32_t *idx,
+                              og_stream stream)
+{
+    g_err[0] = 0;
+    if (!pos || !keys || n == 0 || n >= (1ull << 31) || !(box > 0.0f)) {
+        og_set_error("og_morton_keys: bad argument");
+        return OG_ERR_INVALID_ARG;
+    }
+    OG_CUDA_TRY(ogk_keys(pos, n, box, keys, idx, nullptr, false, (cudaStream_t)stream), return OG_ERR_CUDA);
+    return OG_OK;
+}
+
+extern "C" size_t og_radix_sort_scratch_bytes(uint64_t n) { return ogk_sort_scratch_bytes(n); }
+
+extern "C" int og_radix_sort_pairs(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint32_t *vals_alt,
+                                   uint64_t n, int begin_bit, int end_bit, void *scratch, size_t scratch_bytes,
+                                   int *result_in_alt, og_stream stream)
+{
+    g_err[0] = 0;
+    if (!keys || !vals || !keys_alt || !vals_alt || !scratch || n == 0 || n >= (1ull << 31) || begin_bit < 0 ||
+        end_bit > 64 || begin_bit >= end_bit || scratch_bytes < ogk_sort_scratch_bytes(n)) {
+        og_set_error("og_radix_sort_pairs: bad argument");
+        return OG_ERR_INVALID_ARG;
+    }
+    OG_CUDA_TRY(ogk_radix_sort(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, scratch, result_in_alt,
+                               (cudaStream_t)stream),
+                return OG_ERR_CUDA);
+    return OG_OK;
+}
+
+extern "C" int og_shortrange_accel_host(const float *pos, const float *mass, const float *soft, uint64_t n,
+                                        float box, const og_params *params, const uint32_t *active_idx,
+                                        uint64_t n_active, const float *a_old, float *acc_out, float *pot_out,
+                                        og_stream stream)
+{
+    g_err[0] = 0;
+    if (!check_params(params, n, box)) return OG_ERR_INVALID_ARG;
+    if (!pos || !mass || !soft || !acc_out) { og_set_error("NULL host pointer"); return OG_ERR_INVALID_ARG; }
+    if (!active_idx && n_active != n) { og_set_error("active_idx == NULL requires n_active == n"); return OG_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t na = (size_t)n_active;
+    const size_t o_pos = 0, o_m = o_pos + align_up(n * 12), o_s = o_m + align_up(n * 4), o_ai = o_s + align_up(n * 4),
+                 o_ao = o_ai + align_up(na * 4), o_acc = o_ao + align_up(na * 4), o_pot = o_acc + align_up(na * 12),
+                 total = o_pot + align_up(na * 4);
+    char *d = nullptr;
+    cudaError_t e = cudaMallocAsync((void **)&d, total, st);
+    if (e != cudaSuccess) {
+        og_set_error("cudaMallocAsync(%zu bytes) failed: %s", total, cudaGetErrorString(e));
+        (void)cudaGetLastError();
+        return OG_ERR_OUT_OF_MEMORY;
+    }
+    int rc = OG_OK;
+    og_tree *t = nullptr;
+#define OG_H_TRY(expr) OG_CUDA_TRY(expr, { rc = OG_ERR_CUDA; goto done; })
+    OG_H_TRY(cudaMemcpyAsync(d + o_pos, pos, n * 12, cudaMemcpyHostToDevice, st));
+    OG_H_TRY(cudaMemcpyAsync(d + o_m, mass, n * 4, cudaMemcpyHostToDevice, st));
+    OG_H_TRY(cudaMemcpyAsync(d + o_s, soft, n * 4, cudaMemcpyHostToDevice, st));
+    if (active_idx) OG_H_TRY(cudaMemcpyAsync(d + o_ai, active_idx, na * 4, cudaMemcpyHostToDevice, st));
+    if (a_old) OG_H_TRY(cudaMemcpyAsync(d + o_ao, a_old, na * 4, cudaMemcpyHostToDevice, st));
+    {
+        og_params p = *params;
+        p.workspace = nullptr; p.workspace_bytes = 0;
+        t = og_tree_build((const float *)(d + o_pos), (const float *)(d + o_m), (const float *)(d + o_s), n, box,
+                          &p, stream);
+    }
+    if (!t) { rc = OG_ERR_CUDA; goto done; }
+    rc = og_shortrange_accel(t, active_idx ? (const uint32_t *)(d + o_ai) : nullptr, n_active,
+                             a_old ? (const float *)(d + o_ao) : nullptr, (float *)(d + o_acc),
+                             pot_out ? (float *)(d + o_pot) : nullptr, stream);
+    if (rc != OG_OK) goto done;
+    OG_H_TRY(cudaMemcpyAsync(acc_out, d + o_acc, na * 12, cudaMemcpyDeviceToHost, st));
+    if (pot_out) OG_H_TRY(cudaMemcpyAsync(pot_out, d + o_pot, na * 4, cudaMemcpyDeviceToHost, st));
+    {
+        const int s = og_tree_status(t);  // synchronises
+        if (s != OG_OK) rc = s;
+    }
+#undef OG_H_TRY
+done:
+    if (t) og_tree_free(t, stream);
+    cudaFreeAsync(d, st);
+    cudaStreamSynchronize(st);
+    return rc;
+}
+
+extern "C" int og_ffma_peak_probe(uint64_t iters, double *ms_out, double *flops_out, og_stream stream)
+{
+    g_err[0] = 0;
+    if (!ms_out || !flops_out || iters == 0) { og_set_error("bad argument"); return OG_ERR_INVALID_ARG; }
+    const int sms = device_sm_count(nullptr);
+    if (sms <= 0) { og_set_error("no CUDA device available"); return OG_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)stream;
+    float *sink = nullptr;
+    cudaEvent_t e0, e1;
+    OG_CUDA_TRY(cudaMalloc((void **)&sink, 4096), return OG_ERR_CUDA);
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    int rc = OG_OK;
+    float ms = 0.f;
+    if (ogk_ffma_probe(1000, sms, sink, st) != cudaSuccess) rc = OG_ERR_CUDA;  // warm-up
+    cudaEventRecord(e0, st);
+    if (ogk_ffma_probe(iters, sms, sink, st) != cudaSuccess) rc = OG_ERR_CUDA;
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) rc = OG_ERR_CUDA;
+    cudaEventElapsedTime(&ms, e0, e1);
+    *ms_out = ms;
+    // grid = sms * 8 blocks x 256 threads, 8 chains, 2 flops per FFMA
+    *flops_out = (double)sms * 8.0 * 256.0 * 8.0 * 2.0 * (double)iters;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (rc != OG_OK) og_set_error("ffma probe failed");
+    return rc;
+}

@@ -1,0 +1,114 @@
+// og_internal.cuh -- shared declarations of the CUDA path (sm_100a only).
+// Nothing here is used by, or taken from, oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "og.h"
+
+#define OG_MAX_LEVEL 21
+
+// Latched device-side status bits (og_tree::d_status[0]).
+#define OG_DEV_NODE_OVERFLOW 1u
+#define OG_DEV_BAD_POSITION 2u
+#define OG_DEV_STACK_OVERFLOW 4u
+#define OG_DEV_BAD_INDEX 8u
+
+// Counter slots (og_tree::d_counters), see og_stats.
+enum { OGC_V_FULL = 0, OGC_V_CULL, OGC_A_IN, OGC_P_IN, OGC_P_SOFT, OGC_P_OUT, OGC_FP64, OGC_N };
+
+// Packed node record read by the walk: 4 x float4 + uint2.
+//   com  = (s_x, s_y, s_z, M)                 R9: fp32 rounding of the fp64 upward pass
+//   cell = (c_x, c_y, c_z, l)                 geometric centre and side
+//   lo   = (lo_x, lo_y, lo_z, h_max)          tight AABB (R10: culling only)
+//   hi   = (hi_x, hi_y, hi_z, 0)
+//   info = (start, count | leaf bit)          leaf: first slot / particle count
+//                                             internal: first child / n_child
+#define OG_LEAF_BIT 0x80000000u
+
+struct og_tree {
+    // problem
+    uint64_t n;
+    float box;
+    og_params prm;
+    uint32_t max_nodes;
+    int device;
+    int sm_count;
+    // memory
+    void *arena;            // base of the device allocation (or caller workspace)
+    size_t arena_bytes;
+    int owns_arena;
+    // sorted particles
+    uint64_t *keys;         // sorted keys
+    uint32_t *perm;
+    uint32_t *inv_perm;
+    float4 *spos;           // (x, y, z, m)
+    float *sh;
+    // canonical topology
+    uint8_t *node_level;
+    uint32_t *node_first;
+    uint32_t *node_count;
+    uint32_t *node_first_child;
+    uint8_t *node_nchild;
+    // packed records
+    float4 *node_com;
+    float4 *node_cell;
+    float4 *node_lo;
+    float4 *node_hi;
+    uint2 *node_info;
+    float4 *split_tab;         // OG_NTAB rows (T, dT, E, dE), see walk_math.cuh
+    // small device state
+    uint32_t *d_level_start;   // [24]: start index per level, [22] = n_nodes, [23] = max level
+    uint32_t *d_status;        // [4]: latched status bits, walk work counter, ...
+    unsigned long long *d_counters;  // [OGC_N]
+    // walk scratch (spill stacks), allocated lazily
+    void *walk_spill;
+    size_t walk_spill_bytes;
+    // streams seen
+    cudaStream_t build_stream;
+    mutable cudaStream_t last_stream;
+    mutable int64_t n_nodes_host;   // -1 until read back
+    mutable uint32_t max_level_host;
+};
+
+// ---- error plumbing (api.cu) ----
+void og_set_error(const char *fmt, ...);
+#define OG_CUDA_TRY(expr, onfail)                                                        \
+    do {                                                                                 \
+        cudaError_t _e = (expr);                                                         \
+        if (_e != cudaSuccess) {                                                         \
+            og_set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e),         \
+                         __FILE__, __LINE__);                                            \
+            onfail;                                                                      \
+        }                                                                                \
+    } while (0)
+
+// ---- kernel launchers (one per row of SURVEY.md Sec. 8(a)) ----
+// a1
+cudaError_t ogk_keys(const float *pos, uint64_t n, float box, uint64_t *keys, uint32_t *idx,
+                     uint32_t *d_status, bool validate, cudaStream_t st);
+// a2
+size_t ogk_sort_scratch_bytes(uint64_t n);
+cudaError_t ogk_radix_sort(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint32_t *vals_alt,
+                           uint64_t n, int begin_bit, int end_bit, void *scratch, int *in_alt,
+                           cudaStream_t st);
+// a3
+cudaError_t ogk_gather(const float *pos, const float *mass, const float *soft,
+                       const uint32_t *perm, uint64_t n, float4 *spos, float *sh,
+                       uint32_t *inv_perm, cudaStream_t st);
+// a4 + a5
+size_t ogk_octree_scratch_bytes(uint32_t max_nodes);
+cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st);
+// a6 + a7
+cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out,
+                     uint64_t n_active, const float *a_old, float *acc_out, float *pot_out,
+                     cudaStream_t st);
+size_t ogk_walk_spill_bytes(int sm_count);
+cudaError_t ogk_split_table(float4 *tab, double rcut, double r_s, cudaStream_t st);
+// helpers for the active subset
+cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_perm, uint64_t n,
+                             uint64_t n_active, uint64_t *keys, uint32_t *vals, uint32_t *d_status,
+                             cudaStream_t st);
+cudaError_t ogk_unpack_slots(const uint64_t *keys, uint64_t n_active, uint32_t *slots, cudaStream_t st);
+// misc
+cudaError_t ogk_ffma_probe(uint64_t iters, int sm_count, float *sink, cudaStream_t st);

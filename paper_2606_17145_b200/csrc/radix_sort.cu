@@ -1,0 +1,192 @@
+// radix_sort.cu -- row a2 of SURVEY.md Sec. 8(a): stable LSD radix sort of (u64 key, u32 val)
+// pairs, 8 bits per pass (C2, R3).  Stability is what delivers the index tie-break: the
+// values start as the identity, so equal keys stay in ascending original index.
+//
+// Per pass (HBM-bound): k_hist reads the keys of each 4096-key tile (8 B/key) and writes a
+// per-tile digit histogram; k_scan turns the digit-major histogram into global offsets;
+// k_scatter re-reads the tile (12 B/pair), ranks every key inside its tile in input order
+// (warp match-any ranking, per-warp digit counters in shared memory) and writes the pair to
+// its final place (12 B/pair).  32 B/pair/pass.
+#include "og_internal.cuh"
+
+namespace {
+
+constexpr int SORT_THREADS = 256;
+constexpr int SORT_WARPS = SORT_THREADS / 32;
+constexpr int SORT_ITEMS = 16;                       // keys per thread
+constexpr int SORT_WARP_TILE = 32 * SORT_ITEMS;      // 512 consecutive keys per warp
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS; // 4096 keys per block
+
+__device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
+__device__ __forceinline__ uint32_t lanemask_lt()
+{
+    uint32_t m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// hist[d * n_tiles + tile] = number of keys of the tile whose digit is d; ghist[d] += same.
+__global__ void __launch_bounds__(SORT_THREADS)
+k_sort_hist(const uint64_t *__restrict__ keys, uint64_t n, int shift, uint32_t n_tiles,
+            uint32_t *__restrict__ hist, uint32_t *__restrict__ ghist)
+{
+    __shared__ uint32_t h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    const uint64_t base = (uint64_t)blockIdx.x * SORT_TILE + (threadIdx.x >> 5) * SORT_WARP_TILE + lane_id();
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        const uint64_t i = base + (uint64_t)r * 32;
+        if (i < n) {
+            const uint32_t d = (uint32_t)(__ldg(keys + i) >> shift) & 255u;
+            // aggregate equal digits inside the warp before touching shared memory
+            const uint32_t peers = __match_any_sync(__activemask(), d);
+            if ((peers & lanemask_lt()) == 0) atomicAdd(&h[d], __popc(peers));
+        }
+    }
+    __syncthreads();
+    const uint32_t c = h[threadIdx.x];
+    hist[(uint64_t)threadIdx.x * n_tiles + blockIdx.x] = c;
+    if (c) atomicAdd(&ghist[threadIdx.x], c);
+}
+
+// One block per digit d: exclusive scan of hist[d][0..n_tiles) plus the number of keys with a
+// smaller digit.
+__global__ void __launch_bounds__(1024)
+k_sort_scan(uint32_t *__restrict__ hist, const uint32_t *__restrict__ ghist, uint32_t n_tiles)
+{
+    __shared__ uint32_t warp_sums[32];
+    __shared__ uint32_t carry_s;
+    const uint32_t d = blockIdx.x, tid = threadIdx.x, lane = tid & 31u, wid = tid >> 5;
+    // digit base = sum of ghist[0..d)
+    uint32_t v = (tid < d && tid < 256) ? ghist[tid] : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) warp_sums[wid] = v;
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t s = 0;
+        for (int w = 0; w < 32; ++w) s += warp_sums[w];
+        carry_s = s;
+    }
+    __syncthreads();
+    uint32_t *row = hist + (uint64_t)d * n_tiles;
+    for (uint32_t b0 = 0; b0 < n_tiles; b0 += 1024) {
+        const uint32_t b = b0 + tid;
+        const uint32_t x = (b < n_tiles) ? row[b] : 0;
+        uint32_t incl = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= (uint32_t)o) incl += y;
+        }
+        const uint32_t carry = carry_s;
+        __syncthreads();  // everyone has read carry_s / previous warp_sums
+        if (lane == 31) warp_sums[wid] = incl;
+        __syncthreads();
+        uint32_t woff = 0;
+        for (uint32_t w = 0; w < wid; ++w) woff += warp_sums[w];
+        if (b < n_tiles) row[b] = carry + woff + incl - x;
+        __syncthreads();
+        if (tid == 1023) carry_s = carry + woff + incl;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_sort_scatter(const uint64_t *__restrict__ keys_in, const uint32_t *__restrict__ vals_in,
+               uint64_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out, uint64_t n,
+               int shift, uint32_t n_tiles, const uint32_t *__restrict__ offs)
+{
+    __shared__ uint32_t cnt[SORT_WARPS][256];
+    __shared__ uint32_t gbase[256];
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, wid = tid >> 5;
+#pragma unroll
+    for (int w = 0; w < SORT_WARPS; ++w) cnt[w][tid] = 0;
+    gbase[tid] = offs[(uint64_t)tid * n_tiles + blockIdx.x];
+    __syncthreads();
+
+    const uint64_t base = (uint64_t)blockIdx.x * SORT_TILE + wid * SORT_WARP_TILE + lane;
+    uint64_t key[SORT_ITEMS];
+    uint32_t val[SORT_ITEMS];
+    uint32_t rank[SORT_ITEMS];
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        const uint64_t i = base + (uint64_t)r * 32;
+        const bool ok = i < n;
+        key[r] = ok ? __ldg(keys_in + i) : ~0ull;
+        val[r] = ok ? __ldg(vals_in + i) : 0u;
+    }
+    // rank inside the warp's 512-key chunk, in input order (round-major, lane-minor)
+    const uint32_t lt = lanemask_lt();
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        const bool ok = (base + (uint64_t)r * 32) < n;
+        const uint32_t d = ok ? ((uint32_t)(key[r] >> shift) & 255u) : 256u;
+        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        const int leader = __ffs(peers) - 1;
+        uint32_t b = 0;
+        if ((int)lane == leader && ok) {
+            b = cnt[wid][d];
+            cnt[wid][d] = b + __popc(peers);
+        }
+        b = __shfl_sync(0xffffffffu, b, leader);
+        rank[r] = b + __popc(peers & lt);
+        __syncwarp();
+    }
+    __syncthreads();
+    // exclusive prefix over the warps of the tile, per digit
+    {
+        uint32_t run = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) {
+            const uint32_t c = cnt[w][tid];
+            cnt[w][tid] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        if ((base + (uint64_t)r * 32) < n) {
+            const uint32_t d = (uint32_t)(key[r] >> shift) & 255u;
+            const uint32_t p = gbase[d] + cnt[wid][d] + rank[r];
+            keys_out[p] = key[r];
+            vals_out[p] = val[r];
+        }
+    }
+}
+
+}  // namespace
+
+static inline uint32_t sort_tiles(uint64_t n) { return (uint32_t)((n + SORT_TILE - 1) / SORT_TILE); }
+
+size_t ogk_sort_scratch_bytes(uint64_t n)
+{
+    // per-tile histogram (digit-major) + 8 global histograms
+    return ((size_t)sort_tiles(n) * 256 + 8 * 256) * sizeof(uint32_t) + 256;
+}
+
+cudaError_t ogk_radix_sort(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint32_t *vals_alt,
+                           uint64_t n, int begin_bit, int end_bit, void *scratch, int *in_alt,
+                           cudaStream_t st)
+{
+    const uint32_t n_tiles = sort_tiles(n);
+    uint32_t *hist = reinterpret_cast<uint32_t *>(scratch);
+    uint32_t *ghist = hist + (size_t)n_tiles * 256;
+    const int passes = (end_bit - begin_bit + 7) / 8;
+    cudaError_t e = cudaMemsetAsync(ghist, 0, 8 * 256 * sizeof(uint32_t), st);
+    if (e != cudaSuccess) return e;
+    uint64_t *kin = keys, *kout = keys_alt;
+    uint32_t *vin = vals, *vout = vals_alt;
+    for (int p = 0; p < passes; ++p) {
+        const int shift = begin_bit + 8 * p;
+        k_sort_hist<<<n_tiles, SORT_THREADS, 0, st>>>(kin, n, shift, n_tiles, hist, ghist + 256 * p);
+        k_sort_scan<<<256, 1024, 0, st>>>(hist, ghist + 256 * p, n_tiles);
+        k_sort_scatter<<<n_tiles, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, shift, n_tiles, hist);
+        uint64_t *tk = kin; kin = kout; kout = tk;
+        uint32_t *tv = vin; vin = vout; vout = tv;
+    }
+    if (in_alt) *in_alt = (passes & 1);
+    return cudaGetLastError();
+}

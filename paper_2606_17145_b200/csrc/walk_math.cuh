@@ -1,0 +1,238 @@
+// walk_math.cuh -- per-target arithmetic of the short-range walk (rows a6 of SURVEY.md
+// Sec. 8(a); readings C5, C6, R13..R22 of Sec. 8.3, listed in DESIGN.md Sec. 3).
+//
+// All arithmetic is fp32.  Every *decision* that is discontinuous in the result (open /
+// accept, inside r_cut or not) is taken in fp32 first; if the fp32 operands are within a
+// relative band OG_BAND of the threshold the same test is re-evaluated in fp64 from the same
+// fp32 inputs, in the order the method states it, so that the decision equals the one an
+// exact evaluation takes.  The band is ~30x the worst fp32 error of the
+// tests, and only ~1e-5 of all tests fall inside it.
+#pragma once
+#include "og_internal.cuh"
+
+#define OG_BAND 1.0e-5f
+#define OG_NTAB 1024  // intervals of the split table on [0, r_cut]
+
+struct WalkConst {
+    float L, invL;
+    float rcut, rcut2;
+    float cull_r;        // r_cut * (1 + 1e-5) + 1e-6 L : conservative cull radius
+    float G;
+    float alpha;
+    float theta2;
+    float tab_scale;     // OG_NTAB / r_cut
+    // fp64 copies for the re-evaluation path (C0: fp32 parameters promoted to fp64)
+    double dL, drcut, dG, dalpha, dtheta2;
+};
+
+struct Target {
+    float x, y, z;
+    float h;       // fl32(2.8 eps_i)
+    float A;       // alpha * a_old (fp32 product); unused in geometric mode
+    float aold;    // a_old as given (for the fp64 path)
+    uint32_t slot; // own sorted slot (self exclusion)
+};
+
+struct Accum {
+    float ax, ay, az, pot;
+};
+
+__device__ __forceinline__ float og_wrap(float d, const WalkConst &c)
+{
+    return fmaf(-c.L, rintf(d * c.invL), d);  // R13: d - L round(d / L); exact for |d| < 1.5 L
+}
+
+__device__ __forceinline__ double og_wrap64(double d, double L) { return d - L * round(d / L); }
+
+// (T, dT, E, dE) rows in shared memory: T(w) = erfc(w) + 2w/sqrt(pi) exp(-w^2), E = erfc(w),
+// w = r / (2 r_s), tabulated on r in [0, r_cut] and linearly interpolated (R18).
+__device__ __forceinline__ void og_split(const float4 *__restrict__ tab, float r, const WalkConst &c,
+                                         float &T, float &E)
+{
+    const float t = r * c.tab_scale;
+    int i = (int)t;
+    i = min(i, OG_NTAB - 1);
+    const float f = t - (float)i;
+    const float4 row = tab[i];
+    T = fmaf(f, row.y, row.x);
+    E = fmaf(f, row.w, row.z);
+}
+
+// ---- cutoff decision r < r_cut (R17, strict) ------------------------------------------------
+__device__ __noinline__ bool og_inside_rcut64(float sx, float sy, float sz, const Target &t,
+                                              const WalkConst &c, unsigned long long *counters)
+{
+    const double dx = og_wrap64((double)sx - (double)t.x, c.dL);
+    const double dy = og_wrap64((double)sy - (double)t.y, c.dL);
+    const double dz = og_wrap64((double)sz - (double)t.z, c.dL);
+    const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+    if (counters) atomicAdd(&counters[OGC_FP64], 1ull);
+    return sqrt(r2) < c.drcut;
+}
+
+__device__ __forceinline__ bool og_inside_rcut(float r2, float sx, float sy, float sz, const Target &t,
+                                               const WalkConst &c, unsigned long long *counters)
+{
+    bool in = r2 < c.rcut2;
+    if (fabsf(r2 - c.rcut2) <= OG_BAND * c.rcut2) in = og_inside_rcut64(sx, sy, sz, t, c, counters);
+    return in;
+}
+
+// ---- pair kernel C5 ------------------------------------------------------------------------
+// Source particle (px, py, pz, pm, ph); adds to acc if r < r_cut.  Returns 0 outside, 1 inside
+// with r >= h, 2 inside with r < h.
+template <bool POT>
+__device__ __forceinline__ int og_pair(const float4 p, float ph, const Target &t, const WalkConst &c,
+                                       const float4 *__restrict__ tab, Accum &acc,
+                                       unsigned long long *counters)
+{
+    const float dx = og_wrap(p.x - t.x, c), dy = og_wrap(p.y - t.y, c), dz = og_wrap(p.z - t.z, c);
+    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if (!og_inside_rcut(r2, p.x, p.y, p.z, t, c, counters)) return 0;
+    r2 = fmaxf(r2, 1.0e-36f);           // distinct coincident particles: force 0, potential -14/5 m/h
+    const float rinv = rsqrtf(r2);
+    const float r = r2 * rinv;
+    const float h = fmaxf(t.h, ph);     // R19
+    float T, E;
+    og_split(tab, r, c, T, E);
+    float g, pp;
+    int kind = 1;
+    if (r >= h) {
+        g = rinv * rinv * rinv;
+        pp = -rinv;
+    } else {
+        kind = 2;
+        const float hinv = __frcp_rn(h);
+        const float u = r * hinv, u2 = u * u;
+        const float h3inv = hinv * hinv * hinv;
+        if (u < 0.5f) {
+            g = h3inv * fmaf(u2, fmaf(32.0f, u, -38.4f), 10.666666666666666f);
+            pp = hinv * fmaf(u2, fmaf(u2, fmaf(6.4f, u, -9.6f), 5.333333333333333f), -2.8f);
+        } else {
+            const float uinv = __frcp_rn(u);
+            const float u3inv = uinv * uinv * uinv;
+            g = h3inv * (fmaf(u, fmaf(u, fmaf(-10.666666666666666f, u, 38.4f), -48.0f), 21.333333333333332f) -
+                         0.06666666666666667f * u3inv);
+            pp = hinv * (fmaf(u2, fmaf(u, fmaf(u, fmaf(-2.1333333333333333f, u, 9.6f), -16.0f), 10.666666666666666f),
+                              -3.2f) +
+                         0.06666666666666667f * uinv);
+        }
+    }
+    const float gm = c.G * p.w;
+    const float f = gm * g * T;
+    acc.ax = fmaf(f, dx, acc.ax);
+    acc.ay = fmaf(f, dy, acc.ay);
+    acc.az = fmaf(f, dz, acc.az);
+    if (POT) acc.pot = fmaf(gm * pp, E, acc.pot);
+    return kind;
+}
+
+// ---- node: cull, opening decision, monopole ------------------------------------------------
+struct NodeRec {
+    float4 com;   // s, M
+    float4 cell;  // c, l
+    float4 lo;    // lo, h_max
+    float4 hi;    // hi, -
+};
+
+// Conservative cutoff-box test against the tight AABB (C6 step 1; result-neutral, R17).
+__device__ __forceinline__ bool og_cull(const NodeRec &n, const Target &t, const WalkConst &c)
+{
+    const float mx = 0.5f * (n.lo.x + n.hi.x), my = 0.5f * (n.lo.y + n.hi.y), mz = 0.5f * (n.lo.z + n.hi.z);
+    const float hx = 0.5f * (n.hi.x - n.lo.x), hy = 0.5f * (n.hi.y - n.lo.y), hz = 0.5f * (n.hi.z - n.lo.z);
+    const float ex = fabsf(og_wrap(t.x - mx, c)) - hx;
+    const float ey = fabsf(og_wrap(t.y - my, c)) - hy;
+    const float ez = fabsf(og_wrap(t.z - mz, c)) - hz;
+    return fmaxf(ex, fmaxf(ey, ez)) > c.cull_r;
+}
+
+// fp64 re-evaluation of C6 step 3, exactly in the stated order, from the fp32 inputs.
+template <bool GEOM>
+__device__ __noinline__ bool og_open64(const NodeRec &n, const Target &t, const WalkConst &c,
+                                       unsigned long long *counters)
+{
+    const double x[3] = {(double)t.x, (double)t.y, (double)t.z};
+    const double s[3] = {(double)n.com.x, (double)n.com.y, (double)n.com.z};
+    const double cc[3] = {(double)n.cell.x, (double)n.cell.y, (double)n.cell.z};
+    double d[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) d[k] = og_wrap64(s[k] - x[k], c.dL);
+    const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+    const double M = (double)n.com.w, l = (double)n.cell.w;
+    bool open = false;
+    if (GEOM) {
+        if (__dmul_rn(l, l) > __dmul_rn(c.dtheta2, r2)) open = true;
+    } else {
+        const double A = __dmul_rn(c.dalpha, (double)t.aold);
+        if (__dmul_rn(__dmul_rn(__dmul_rn(c.dG, M), l), l) > __dmul_rn(__dmul_rn(A, r2), r2)) open = true;
+    }
+    bool inside = true;
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        if (!(fabs(og_wrap64(cc[k] - x[k], c.dL)) < __dmul_rn(0.6, l))) inside = false;
+    if (inside) open = true;
+    const double hm = (double)n.lo.w, hi = (double)t.h;
+    const double hh = hi > hm ? hi : hm;
+    if (r2 < __dmul_rn(hh, hh)) open = true;
+    if (counters) atomicAdd(&counters[OGC_FP64], 1ull);
+    return open;
+}
+
+// C6 steps 2-3 in fp32 (+ band re-evaluation).  Outputs d = wrap(s - x) and r2.
+template <bool GEOM>
+__device__ __forceinline__ bool og_open(const NodeRec &n, const Target &t, const WalkConst &c, float &dx,
+                                        float &dy, float &dz, float &r2, unsigned long long *counters)
+{
+    dx = og_wrap(n.com.x - t.x, c);
+    dy = og_wrap(n.com.y - t.y, c);
+    dz = og_wrap(n.com.z - t.z, c);
+    r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const float l = n.cell.w;
+    const float l2 = l * l;
+    float lhs, rhs;
+    if (GEOM) {
+        lhs = l2;
+        rhs = c.theta2 * r2;
+    } else {
+        lhs = c.G * n.com.w * l2;   // R14: G M l^2 > alpha a_old r^4, strict
+        rhs = t.A * r2 * r2;
+    }
+    bool open = lhs > rhs;
+    bool amb = fabsf(lhs - rhs) <= OG_BAND * fmaxf(lhs, rhs);
+    // inside guard R15: |wrap(c_k - x_k)| < 0.6 l for all k
+    const float lim = 0.6f * l;
+    const float cx = fabsf(og_wrap(n.cell.x - t.x, c)), cy = fabsf(og_wrap(n.cell.y - t.y, c)),
+                cz = fabsf(og_wrap(n.cell.z - t.z, c));
+    const float cmax = fmaxf(cx, fmaxf(cy, cz));
+    open |= cmax < lim;
+    // only the largest component can sit on the threshold in a way that matters
+    amb |= fabsf(cmax - lim) <= OG_BAND * l;
+    // softening guard R16: r^2 < max(h_i, h_max)^2
+    const float hh = fmaxf(t.h, n.lo.w);
+    const float hh2 = hh * hh;
+    open |= r2 < hh2;
+    amb |= fabsf(r2 - hh2) <= OG_BAND * hh2;
+    if (amb) open = og_open64<GEOM>(n, t, c, counters);
+    return open;
+}
+
+// C6 step 4: accepted node, Newtonian monopole times the split factor (R21).  Returns 1 if
+// r < r_cut.
+template <bool POT>
+__device__ __forceinline__ int og_monopole(const NodeRec &n, const Target &t, const WalkConst &c,
+                                           const float4 *__restrict__ tab, float dx, float dy, float dz,
+                                           float r2, Accum &acc, unsigned long long *counters)
+{
+    if (!og_inside_rcut(r2, n.com.x, n.com.y, n.com.z, t, c, counters)) return 0;
+    const float rinv = rsqrtf(r2);
+    const float r = r2 * rinv;
+    float T, E;
+    og_split(tab, r, c, T, E);
+    const float gm = c.G * n.com.w;
+    const float f = gm * T * rinv * rinv * rinv;
+    acc.ax = fmaf(f, dx, acc.ax);
+    acc.ay = fmaf(f, dy, acc.ay);
+    acc.az = fmaf(f, dz, acc.az);
+    if (POT) acc.pot = fmaf(-gm * rinv, E, acc.pot);
+    return 1;
+}
