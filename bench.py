@@ -1,0 +1,406 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line per run (contract in the task statement).
+
+    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload nfw256]
+
+A "step" is one pass of the whole hot path over one batch of
+synthetic input: og_tree_build (Morton keys -> radix sort -> gather -> octree -> upward pass)
+followed by og_shortrange_accel (relative opening criterion, alpha = 0.005, a_old from an untimed
+geometric-theta pass) on all active targets.  Default workload: BASELINE.json configs[2], the
+16.8M-particle clustered box the north_star's roofline target is quoted on ("nfw256").
+
+value    = active particles per second over the whole step, inputs resident in HBM.
+e2e      = the same through og_shortrange_accel_host with pinned HOST buffers (H2D + D2H inside).
+roofline = the walk kernel (dominant): algorithmic flops (oracle-counted per-target figure of
+           paper_2606_17145_b200/algorithmic_units.json x active targets) / its CUDA-event time,
+           against the FP32 ALU peak SMs x 128 lanes x 2 flop x max SM clock ("bound": "alu").
+cpu_baseline = the oracle (oracle/, untuned) on the host cores, bounded sample, rank 0, N = 1.
+
+N > 1: one process per GPU (torchrun); every rank works on its own seeded box of the same config
+(weak scaling, no data-path collective -- DESIGN.md Sec. 8); time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_17145_b200 import workloads as W  # noqa: E402
+
+METRIC = "short-range tree-gravity particles/s (tree build + walk, 1 step) on B200"
+UNIT = "particles/s"
+SM_LANES = 128          # FP32 lanes per SM (B200)
+KERNELS_PER_BUILD = 1 + 8 * 3 + 1 + 1 + 2   # keys, 8 x (hist, scan, scatter), gather, split table, octree + upward
+KERNELS_PER_WALK_ALL = 1
+
+
+def load_units(name):
+    p = os.path.join(ROOT, "paper_2606_17145_b200", "algorithmic_units.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        return json.load(f).get(name)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        for ts, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                if t0 - 0.05 <= ts <= t1 + 0.15:
+                    sm.append(float(f[0]))
+                smax = float(f[1])
+            except ValueError:
+                continue
+            if t0 - 0.05 <= ts <= t1 + 0.15:
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def make_workload(name, rank):
+    """BASELINE.json config by name; rank r > 0 draws an independent box with seed + 7919 r."""
+    if rank == 0:
+        return W.make(name)
+    if name == "nfw256":
+        return W.nfw_box(256, 2000, 100.0, W.SEED0 + 3000 + 7919 * rank)
+    if name == "uniform32":
+        return W.uniform_box(32, 1.0, W.SEED0 + 1000 + 7919 * rank)
+    if name == "lattice128":
+        return W.perturbed_lattice(128, 1.0, W.SEED0 + 2000 + 7919 * rank)
+    if name == "zoom":
+        return W.zoom(seed=W.SEED0 + 4000 + 7919 * rank)
+    return W.make(name)
+
+
+def aggregate(n_active_per_rank, ms_max):
+    """value over all ranks: units all ranks processed / max-over-ranks time."""
+    return float(sum(n_active_per_rank)) / (ms_max * 1e-3)
+
+
+def dist_setup(n_gpus, backend):
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group(backend=backend)
+    return world, rank, local
+
+
+def all_max(x, device):
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return x
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def all_gather_int(x, device):
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return [x]
+    t = torch.tensor([x], dtype=torch.int64, device=device)
+    out = [torch.zeros_like(t) for _ in range(dist.get_world_size())]
+    dist.all_gather(out, t)
+    return [int(o.item()) for o in out]
+
+
+def barrier():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        dist.barrier()
+
+
+def cpu_baseline(w, sample=1 << 17, seed=4242):
+    """The oracle as it stands on the host cores: full tree build (single thread) + relative-criterion walk
+    of a seeded random sample of the active targets (all cores), walk time scaled to all active targets."""
+    import oracle
+    prm = oracle.make_params(w.L, w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta)
+    t0 = time.perf_counter()
+    t = oracle.build_tree(w.pos, w.mass, w.eps, prm)
+    t_build = time.perf_counter() - t0
+    act = np.arange(w.n, dtype=np.uint32) if w.active_idx is None else w.active_idx
+    rng = np.random.Generator(np.random.PCG64(seed))
+    ns = min(sample, act.shape[0])
+    sub = np.sort(rng.choice(act, ns, replace=False)).astype(np.uint32)
+    a1, _, _ = oracle.walk(t, sub, None, want_counters=False)          # a_old (untimed, as on the GPU)
+    a_old = np.linalg.norm(a1, axis=1).astype(np.float32)
+    t0 = time.perf_counter()
+    oracle.walk(t, sub, a_old, want_counters=False)
+    t_walk = time.perf_counter() - t0
+    t_full = t_build + t_walk * (act.shape[0] / ns)
+    return {"value": act.shape[0] / t_full, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"full {w.n}-particle oracle tree build ({t_build:.1f} s, 1 thread) + relative-criterion walk of "
+                      f"{ns} seeded random targets ({t_walk:.2f} s on {oracle.num_threads()} threads), walk time scaled "
+                      f"by {act.shape[0]}/{ns}",
+            "build_s": t_build, "walk_sample_s": t_walk, "walk_us_per_target_per_core":
+            1e6 * t_walk * oracle.num_threads() / ns}, t
+
+
+def run_reference(args):
+    """--impl reference: the oracle, timed on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    w = W.make(args.workload)
+    prm = oracle.make_params(w.L, w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta)
+    t0 = time.perf_counter()
+    t = oracle.build_tree(w.pos, w.mass, w.eps, prm)
+    t_build = time.perf_counter() - t0
+    act = np.arange(w.n, dtype=np.uint32) if w.active_idx is None else w.active_idx
+    ns = min(args.ref_sample, act.shape[0])
+    times = []
+    for it in range(args.warmup + args.steps):
+        rng = np.random.Generator(np.random.PCG64(977 + it))
+        sub = np.sort(rng.choice(act, ns, replace=False)).astype(np.uint32)
+        a1, _, _ = oracle.walk(t, sub, None, want_counters=False)
+        a_old = np.linalg.norm(a1, axis=1).astype(np.float32)
+        t0 = time.perf_counter()
+        oracle.walk(t, sub, a_old, want_counters=False)
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            times.append(dt)
+    t_walk = float(np.mean(times))
+    t_full = t_build + t_walk * (act.shape[0] / ns)
+    value = act.shape[0] / t_full
+    sample = (f"per step: relative-criterion oracle walk of {ns} seeded random targets, scaled by {act.shape[0]}/{ns}, "
+              f"plus the full {w.n}-particle oracle tree build measured once ({t_build:.1f} s, 1 thread)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_full, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "n": w.n, "n_active": w.n_active},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    from paper_2606_17145_b200 import binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    world, rank, local = dist_setup(args.gpus, "nccl")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    w = make_workload(args.workload, rank)
+    n, na = w.n, w.n_active
+    prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8)
+    h_pos = torch.from_numpy(w.pos).pin_memory()
+    h_mass = torch.from_numpy(w.mass).pin_memory()
+    h_eps = torch.from_numpy(w.eps).pin_memory()
+    h_act = None if w.active_idx is None else torch.from_numpy(w.active_idx.view(np.int32)).pin_memory()
+    pos, mass, eps = h_pos.to(dev), h_mass.to(dev), h_eps.to(dev)
+    act = None if h_act is None else h_act.to(dev)
+    acc = torch.empty((na, 3), dtype=torch.float32, device=dev)
+    pot = torch.empty((na,), dtype=torch.float32, device=dev)
+
+    # a_old: |a| of a geometric-theta pass (R23), untimed
+    tree = B.og_tree_build(pos, mass, eps, w.L, prm)
+    B.og_shortrange_accel(tree, act, None, acc_out=acc, pot_out=pot)
+    a_old = torch.linalg.vector_norm(acc, dim=1).contiguous()
+    if B.og_tree_status(tree) != B.OG_OK:
+        raise SystemExit("bench.py: tree status " + B.og_last_error())
+    st_tree = B.og_tree_stats(tree)
+    B.og_tree_free(tree)
+
+    def step(ev=None):
+        if ev:
+            ev[0].record()
+        t = B.og_tree_build(pos, mass, eps, w.L, prm)
+        if ev:
+            ev[1].record()
+        B.og_shortrange_accel(t, act, a_old, acc_out=acc, pot_out=pot)
+        if ev:
+            ev[2].record()
+        B.og_tree_free(t)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    barrier()
+    torch.cuda.synchronize()
+    t0 = time.time()
+    e0.record()
+    for k in range(args.steps):
+        step(evs[k])
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    t1 = time.time()
+    ms_total = all_max(e0.elapsed_time(e1), dev)
+    clocks = sampler.stop(t0, t1)
+    ms_step = ms_total / args.steps
+    ms_build = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    ms_walk = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    n_act_all = all_gather_int(na, dev)
+    value = aggregate(n_act_all, ms_step)
+
+    # e2e through the HOST-buffer entry point (pinned inputs, H2D + build + walk + D2H inside)
+    h_aold = a_old.cpu().pin_memory()
+    h_acc = torch.empty((na, 3), dtype=torch.float32).pin_memory()
+    h_pot = torch.empty((na,), dtype=torch.float32).pin_memory()
+    e2e_steps = max(1, min(args.steps, 3))
+    B.og_shortrange_accel_host(h_pos, h_mass, h_eps, w.L, prm, h_act, h_aold, acc_out=h_acc, pot_out=h_pot)
+    barrier()
+    torch.cuda.synchronize()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record()
+    for _ in range(e2e_steps):
+        B.og_shortrange_accel_host(h_pos, h_mass, h_eps, w.L, prm, h_act, h_aold, acc_out=h_acc, pot_out=h_pot)
+    f1.record()
+    torch.cuda.synchronize()
+    ms_e2e = all_max(f0.elapsed_time(f1), dev) / e2e_steps
+    h2d = n * 20 + na * 4 + (0 if h_act is None else na * 4)
+    d2h = na * 16
+
+    if rank != 0:
+        return 0
+    # counters of one untimed counted walk (cross-check of the oracle-counted per-target figure)
+    prm_c = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8,
+                          flags=B.OG_PERIODIC | B.OG_COUNT)
+    tc = B.og_tree_build(pos, mass, eps, w.L, prm_c)
+    B.og_shortrange_accel(tc, act, a_old, acc_out=acc, pot_out=pot)
+    stc = B.og_tree_stats(tc)
+    status = B.og_tree_status(tc)
+    B.og_tree_free(tc)
+    checksum = float(torch.linalg.vector_norm(acc.double(), dim=1).mean().item())
+
+    peaks, peaks_src = measured_peaks()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    fmax = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    peak_tflops = sms * SM_LANES * 2 * fmax / 1e12
+    units = load_units(w.name)
+    Wt = {"V_cull": 6, "V_full": 16, "A_in": 21, "P_out": 11, "P_in": 32, "P_soft_extra": 13}
+    F_gpu = (Wt["V_cull"] * stc["V_cull"] + Wt["V_full"] * stc["V_full"] + Wt["A_in"] * stc["A_in"] +
+             Wt["P_out"] * stc["P_out"] + Wt["P_in"] * stc["P_in"] + Wt["P_soft_extra"] * stc["P_soft"])
+    if units:
+        F_alg = units["F_alg_per_target"] * na
+        F_int = units["F_int_per_target"] * na
+        inter = units["interactions_per_target"] * na
+        units_src = "oracle-counted per-target figure (algorithmic_units.json) x active targets"
+    else:
+        F_alg, F_int, inter = float(F_gpu), None, float(stc["A_in"] + stc["P_in"])
+        units_src = "GPU OG_COUNT counters (no oracle figure for this workload)"
+    achieved = F_alg / (ms_walk * 1e-3) / 1e12
+    ffma_ms, ffma_fl = B.og_ffma_peak_probe(100000)
+    t_hbm_ms = (units["compulsory_hbm_bytes"] if units else 0) / (float(peaks["hbm_gbs"]) * 1e9) * 1e3
+    roofline = {
+        "bound": "alu", "kernel": "k_walk_group", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": achieved / peak_tflops, "traffic": None,
+        "peak_source": f"{sms} SMs x {SM_LANES} FP32 lanes x 2 flop x {fmax / 1e6:.0f} MHz (max SM clock, "
+                       f"MEASURED_PEAKS.json {peaks_src}); DESIGN.md Sec. 7",
+        "algorithmic_flops_per_launch": F_alg, "units": units_src,
+        "frac_interactions_only": (F_int / (ms_walk * 1e-3) / 1e12 / peak_tflops) if F_int else None,
+        "algorithmic_flops_gpu_counters": float(F_gpu),
+        "ffma_probe_tflops": ffma_fl / (ffma_ms * 1e-3) / 1e12,
+        "hbm_bound_ms": t_hbm_ms, "alu_bound_ms": F_alg / (peak_tflops * 1e12) * 1e3,
+        "kernel_ms": ms_walk, "kernel_share_of_step": ms_walk / (ms_build + ms_walk),
+    }
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": w.name, "n": n, "n_active": na, "box": w.L, "r_s": w.r_s, "alpha": w.alpha,
+                   "leaf_max": 8, "n_nodes": st_tree["n_nodes"], "max_level": st_tree["max_level"],
+                   "l2_policy": "inputs larger than L2 (no flush): particles + tree > 1.5 GB vs 126 MB L2",
+                   "parallelism": f"{world} independent boxes (one per GPU)" if world > 1 else "1 GPU"},
+        "clocks": clocks,
+        "e2e": {"value": aggregate(n_act_all, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e, "steps": e2e_steps},
+        "gpu_launches": args.steps * (KERNELS_PER_BUILD + KERNELS_PER_WALK_ALL + (0 if act is None else 2 + 3 * 4)),
+        "roofline": roofline,
+        "breakdown_ms": {"build_a1_a5": ms_build, "walk_a6_a7": ms_walk},
+        "particles_per_s_walk_only": na / (ms_walk * 1e-3),
+        "interactions_per_s_walk_only": inter / (ms_walk * 1e-3),
+        "walk_counters": stc, "status": status, "checksum_mean_abs_acc": checksum,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        cb, _ = cpu_baseline(w, sample=args.cpu_sample)
+        line["cpu_baseline"] = cb
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="nfw256", choices=list(W.CONFIG_NAMES))
+    ap.add_argument("--cpu-sample", type=int, default=1 << 17)
+    ap.add_argument("--ref-sample", type=int, default=1 << 15)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3 if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

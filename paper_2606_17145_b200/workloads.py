@@ -109,7 +109,7 @@ def perturbed_lattice(n_side: int = 128, L: float = 1.0, seed: int = SEED0 + 200
     dk[:, :, nyq] = 0.0
     psi = []
     for K in (KX, KY, KZ):
-        psi.append(np.fft.irfftn(1j * K * dk / k2, s=(n, n, n)))
+        psi.append(np.fft.irfftn(1j * K * dk / k2, s=(n, n, n), axes=(0, 1, 2)))
     psi = np.stack(psi, axis=-1).reshape(-1, 3)
     rms3 = np.sqrt(np.mean(np.sum(psi * psi, axis=1)))
     psi *= (rms_cells * L / n) / rms3
