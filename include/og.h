@@ -84,6 +84,10 @@ typedef struct {
     uint64_t P_soft;        /* ... of which r < h                                          */
     uint64_t P_out;         /* particle pairs evaluated with r >= r_cut                    */
     uint64_t fp64_rechecks; /* decisions re-evaluated in fp64           */
+    /* group-walk diagnostics (OG_COUNT): nodes classified at group level as dropped / opened by
+     * all / accepted by all / undecided; particles dropped / staged shifted / staged for per-lane
+     * wrap; node batches popped                                                              */
+    uint64_t cl_drop, cl_open, cl_accept, cl_generic, pt_drop, pt_shift, pt_wrap, batches;
 } og_stats;
 
 /* og_tree_get field selectors.  Pointers are DEVICE pointers into the tree, valid until

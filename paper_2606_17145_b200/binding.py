@@ -59,7 +59,10 @@ class og_params(C.Structure):
 class og_stats(C.Structure):
     _fields_ = [("n", C.c_uint64), ("n_nodes", C.c_uint64), ("max_level", C.c_uint32), ("reserved", C.c_uint32),
                 ("V_full", C.c_uint64), ("V_cull", C.c_uint64), ("A_in", C.c_uint64), ("P_in", C.c_uint64),
-                ("P_soft", C.c_uint64), ("P_out", C.c_uint64), ("fp64_rechecks", C.c_uint64)]
+                ("P_soft", C.c_uint64), ("P_out", C.c_uint64), ("fp64_rechecks", C.c_uint64),
+                ("cl_drop", C.c_uint64), ("cl_open", C.c_uint64), ("cl_accept", C.c_uint64),
+                ("cl_generic", C.c_uint64), ("pt_drop", C.c_uint64), ("pt_shift", C.c_uint64),
+                ("pt_wrap", C.c_uint64), ("batches", C.c_uint64)]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}

@@ -47,7 +47,7 @@ Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count)
     L.level_start = take(24 * 4);
     L.status = take(16 * 4);
     L.counters = take(OGC_N * 8);
-    L.split_tab = take(1024 * 16);
+    L.split_tab = take(1025 * 16);
     L.spill = take(ogk_walk_spill_bytes(sm_count));
     L.total = o;
     return L;
@@ -302,6 +302,9 @@ extern "C" int og_tree_stats(const og_tree *t, og_stats *out)
     out->V_full = c[OGC_V_FULL]; out->V_cull = c[OGC_V_CULL]; out->A_in = c[OGC_A_IN];
     out->P_in = c[OGC_P_IN]; out->P_soft = c[OGC_P_SOFT]; out->P_out = c[OGC_P_OUT];
     out->fp64_rechecks = c[OGC_FP64];
+    out->cl_drop = c[OGC_CL_DROP]; out->cl_open = c[OGC_CL_OPEN]; out->cl_accept = c[OGC_CL_ACCEPT];
+    out->cl_generic = c[OGC_CL_GENERIC]; out->pt_drop = c[OGC_PT_DROP]; out->pt_shift = c[OGC_PT_SHIFT];
+    out->pt_wrap = c[OGC_PT_WRAP]; out->batches = c[OGC_BATCHES];
     return OG_OK;
 }
 

@@ -6,13 +6,16 @@
 // consecutive in Morton order.  The warp traverses the UNION of its lanes' walks, but every
 // lane accepts / opens exactly the nodes its own serial walk would (C6): each pending entry
 // carries a 32-bit lane mask = the lanes that opened the parent.  Per iteration the warp pops
-// up to 32 child nodes from a shared-memory stack of (first, count, mask) ranges, lane k
-// loads node k (4 x LDG.128, children are contiguous), the records are staged in shared
-// memory, every lane scans the staged batch (broadcast LDS.128) doing cull / opening test /
-// monopole for the entries whose mask holds its bit, and a ballot per entry yields the mask
-// of the children.  Opened leaves go to a second range list whose particles are staged and
-// evaluated the same way in batches of 32.  The split table (T, dT, E, dE) lives in shared
-// memory.  Results are written straight to the caller's order (a7 fused).
+// up to 32 child nodes from a shared-memory stack of (first, count, mask) ranges and lane k
+// loads node k (4 x LDG.128, children are contiguous) and classifies it against the GROUP
+// (bounding box of the 32 targets, range of a_old, largest h): dropped by the cutoff box,
+// opened by every target, accepted by every target, or undecided.  Only the last two classes
+// are staged in shared memory and scanned by all lanes (broadcast LDS.128): accepted-by-all
+// nodes cost one monopole per lane with no decision work, undecided ones get the exact
+// per-lane cull / opening test and a ballot yields the mask of the children.  Opened leaves go
+// to a second range list whose particles are staged (after a group-level cutoff test and an
+// exact periodic shift) and evaluated in batches of 32.  The split table (T, T', E, E') lives in
+// shared memory.  Results are written straight to the caller's order (a7 fused).
 //
 // k_walk_simple: one thread per target with a private stack; debugging / comparison only.
 #include "walk_math.cuh"
@@ -66,7 +69,7 @@ __device__ __forceinline__ Target load_target(const WalkArgs &a, uint32_t k, uin
 
 __device__ __forceinline__ void copy_table(float4 *s_tab, const float4 *g_tab)
 {
-    for (int i = threadIdx.x; i < OG_NTAB; i += blockDim.x) s_tab[i] = g_tab[i];
+    for (int i = threadIdx.x; i < OG_NTAB + 1; i += blockDim.x) s_tab[i] = g_tab[i];
 }
 
 // -------------------------------------------------------------------------------------------
@@ -74,7 +77,7 @@ template <bool GEOM, bool POT, bool COUNT>
 __global__ void __launch_bounds__(128)
 k_walk_simple(WalkArgs a)
 {
-    __shared__ float4 s_tab[OG_NTAB];
+    __shared__ float4 s_tab[OG_NTAB + 1];
     copy_table(s_tab, a.tab);
     __syncthreads();
     const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -129,16 +132,20 @@ k_walk_simple(WalkArgs a)
 // -------------------------------------------------------------------------------------------
 constexpr int GW_WARPS = 8;           // warps per block
 constexpr int GW_THREADS = GW_WARPS * 32;
-constexpr int GW_STACK = 384;         // node-range stack entries per warp in shared memory
-constexpr int GW_SPILL = 192;         // entries moved to / from global memory at a time
+constexpr int GW_STACK = 256;         // node-range stack entries per warp in shared memory
+constexpr int GW_SPILL = 128;         // entries moved to / from global memory at a time
 constexpr int GW_PLIST = 64;          // particle-range list entries per warp
 
 struct __align__(16) WarpSmem {
-    float4 nd_com[32], nd_cell[32], nd_lo[32], nd_hi[32];
-    float4 pt_pos[32];
+    float4 xn_com[32], xn_aux[32];                          // class X (per-lane decision): (s', GM), (lhs, near2, cull2, wrap)
+    uint32_t xn_idx[32];
+    float4 an_com[32];                                      // class A (accepted by all) nodes: (s', GM)
+    float4 pt_pos[32];                                      // staged particles (x', y', z', m)
     float pt_h[32];
     uint32_t pt_slot[32];
-    uint32_t bt_mask[32];             // masks of the staged batch (nodes or particles)
+    uint32_t pt_mask[32];             // bit 31.. : lane masks; pt_flag: generic (per-lane wrap) or shifted
+    uint32_t pt_flag[32];
+    uint32_t xn_mask[32], an_mask[32];
     uint32_t st_start[GW_STACK], st_cnt[GW_STACK], st_mask[GW_STACK];
     uint32_t pl_start[GW_PLIST], pl_cnt[GW_PLIST], pl_mask[GW_PLIST];
 };
@@ -181,33 +188,167 @@ __device__ __forceinline__ uint32_t pop_items(uint32_t *s_start, uint32_t *s_cnt
     return total;
 }
 
+// Warp-uniform description of the 32 targets of a group: bounding box (centre, half size), range
+// of a_old, largest softening length.
+struct GroupInfo {
+    float gcx, gcy, gcz, ghx, ghy, ghz;
+    float amin, amax, hmax;
+};
+
+enum { CL_DROP = 0, CL_OPEN = 1, CL_ACCEPT = 2, CL_GENERIC = 3 };
+
+#define OG_GM 1.0e-4f   // relative safety margin of the group-level (conservative) classifications
+
+// Group-level classification of one node by the lane that loaded it.  Every
+// outcome other than CL_GENERIC is one that EVERY target of the group would reach on its own:
+//   CL_DROP    no target can be within r_cut of the node's AABB (cutoff-box test, result-neutral), or
+//              all accept it but none is within r_cut of its centre of mass;
+//   CL_OPEN    every target opens it (relative / geometric criterion at the largest possible r and
+//              a_old, or the group lies inside the 0.6 l guard box, or inside the softening guard);
+//   CL_ACCEPT  every target accepts it (criterion at the smallest possible r and a_old, no guard can
+//              fire) and one exact periodic shift serves all targets: `sc` = (s - k L, G M).
+template <bool GEOM>
+__device__ __forceinline__ int classify_node(const NodeRec &n, const GroupInfo &g, const WalkConst &c, float4 &sc,
+                                             float4 &aux)
+{
+    const float l = n.cell.w;
+    // cutoff box against the group's bounding box
+    const float gapx = fabsf(og_wrap(0.5f * (n.lo.x + n.hi.x) - g.gcx, c)) - 0.5f * (n.hi.x - n.lo.x) - g.ghx;
+    const float gapy = fabsf(og_wrap(0.5f * (n.lo.y + n.hi.y) - g.gcy, c)) - 0.5f * (n.hi.y - n.lo.y) - g.ghy;
+    const float gapz = fabsf(og_wrap(0.5f * (n.lo.z + n.hi.z) - g.gcz, c)) - 0.5f * (n.hi.z - n.lo.z) - g.ghz;
+    if (fmaxf(gapx, fmaxf(gapy, gapz)) > c.cull_r) return CL_DROP;
+    // distance range |s - x| over the group's box, per axis (valid on the periodic circle)
+    const float kx = rintf((n.com.x - g.gcx) * c.invL), ky = rintf((n.com.y - g.gcy) * c.invL),
+                kz = rintf((n.com.z - g.gcz) * c.invL);
+    const float adx = fabsf(fmaf(-c.L, kx, n.com.x - g.gcx)), ady = fabsf(fmaf(-c.L, ky, n.com.y - g.gcy)),
+                adz = fabsf(fmaf(-c.L, kz, n.com.z - g.gcz));
+    const float nx = fmaxf(adx - g.ghx, 0.f), ny = fmaxf(ady - g.ghy, 0.f), nz = fmaxf(adz - g.ghz, 0.f);
+    const float fx = adx + g.ghx, fy = ady + g.ghy, fz = adz + g.ghz;
+    const float rmin2 = fmaf(nz, nz, fmaf(ny, ny, nx * nx));
+    const float rmax2 = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
+    const float l2 = l * l;
+    const float GM = c.G * n.com.w;
+    float lhs, rhs_max, rhs_min;
+    if (GEOM) {
+        lhs = l2; rhs_max = c.theta2 * rmax2; rhs_min = c.theta2 * rmin2;
+    } else {
+        lhs = GM * l2;
+        rhs_max = c.alpha * g.amax * rmax2 * rmax2;
+        rhs_min = c.alpha * g.amin * rmin2 * rmin2;
+    }
+    if (lhs > rhs_max * (1.0f + OG_GM)) return CL_OPEN;
+    // inside guard R15 at group level: offsets of the group's box from the cell centre, per axis
+    const float icx = fabsf(og_wrap(n.cell.x - g.gcx, c)), icy = fabsf(og_wrap(n.cell.y - g.gcy, c)),
+                icz = fabsf(og_wrap(n.cell.z - g.gcz, c));
+    if (fmaxf(icx + g.ghx, fmaxf(icy + g.ghy, icz + g.ghz)) < 0.6f * l * (1.0f - OG_GM)) return CL_OPEN;   // all inside
+    if (rmax2 < n.lo.w * n.lo.w * (1.0f - OG_GM)) return CL_OPEN;                       // R16 fires for all
+    // no target can be inside the guard box if the group's box misses it on some axis
+    const bool no_inside = fmaxf(icx - g.ghx, fmaxf(icy - g.ghy, icz - g.ghz)) > 0.6f * l * (1.0f + OG_GM);
+    const float hh = fmaxf(g.hmax, n.lo.w);
+    const bool no_guard = no_inside && rmin2 > hh * hh * (1.0f + OG_GM);
+    // one periodic image for all targets, and s - k L exact (k = 0, or k = +1 with s >= L/2)
+    const bool shifted = fmaxf(fx, fmaxf(fy, fz)) < 0.5f * c.L * (1.0f - OG_GM) && fminf(kx, fminf(ky, kz)) >= 0.0f;
+    if (shifted) sc = make_float4(fmaf(-c.L, kx, n.com.x), fmaf(-c.L, ky, n.com.y), fmaf(-c.L, kz, n.com.z), GM);
+    else sc = make_float4(n.com.x, n.com.y, n.com.z, GM);
+    if (no_guard && lhs < rhs_min * (1.0f - OG_GM)) {
+        if (rmin2 > c.rcut2 * (1.0f + OG_GM)) return CL_DROP;
+        if (shifted) return CL_ACCEPT;
+    }
+    // undecided: what the per-lane fast test needs.  near2 = below this r^2 a guard could fire and the exact
+    // test is taken; cull2 = (r_cut + R)^2 with R = largest distance from s to a corner of the AABB.
+    const float ex = fmaxf(n.com.x - n.lo.x, n.hi.x - n.com.x), ey = fmaxf(n.com.y - n.lo.y, n.hi.y - n.com.y),
+                ez = fmaxf(n.com.z - n.lo.z, n.hi.z - n.com.z);
+    const float R = sqrtf(fmaf(ez, ez, fmaf(ey, ey, ex * ex))) * (1.0f + OG_GM);
+    const float rc = c.cull_r + R;
+    const float near2 = fmaxf(no_inside ? 0.0f : 3.7f * l2, n.lo.w * n.lo.w * (1.0f + OG_GM));
+    aux = make_float4(lhs, near2, rc * rc, shifted ? 0.0f : 1.0f);
+    return CL_GENERIC;
+}
+
+// Exact per-lane visit of one node from its full record (cull, opening test with fp64 band, monopole).
+// Out of line: taken only by the few (lane, node) pairs the fast test cannot settle.
+template <bool GEOM, bool POT>
+__device__ __noinline__ bool slow_visit(const WalkArgs &a, uint32_t node, const Target &t, const float4 *s_tab,
+                                        Accum &acc, unsigned long long *cnt, uint32_t &n_in)
+{
+    const NodeRec m = load_node(a, node);
+    if (og_cull(m, t, a.c)) return false;
+    float dx, dy, dz, r2;
+    if (og_open<GEOM>(m, t, a.c, dx, dy, dz, r2, cnt)) return true;
+    n_in += og_monopole<POT>(m, t, a.c, s_tab, dx, dy, dz, r2, acc, cnt);
+    return false;
+}
+
+// Group-level treatment of one particle by the lane that loaded it: 0 = no target within r_cut
+// (dropped), 1 = staged with one exact periodic shift for all targets, 2 = staged as is (per-lane wrap).
+__device__ __forceinline__ int classify_particle(float4 &p, const GroupInfo &g, const WalkConst &c)
+{
+    const float kx = rintf((p.x - g.gcx) * c.invL), ky = rintf((p.y - g.gcy) * c.invL), kz = rintf((p.z - g.gcz) * c.invL);
+    const float adx = fabsf(fmaf(-c.L, kx, p.x - g.gcx)), ady = fabsf(fmaf(-c.L, ky, p.y - g.gcy)),
+                adz = fabsf(fmaf(-c.L, kz, p.z - g.gcz));
+    const float nx = fmaxf(adx - g.ghx, 0.f), ny = fmaxf(ady - g.ghy, 0.f), nz = fmaxf(adz - g.ghz, 0.f);
+    if (fmaf(nz, nz, fmaf(ny, ny, nx * nx)) > c.rcut2 * (1.0f + OG_GM)) return 0;
+    const float halfL = 0.5f * c.L * (1.0f - OG_GM);
+    if (fmaxf(adx + g.ghx, fmaxf(ady + g.ghy, adz + g.ghz)) < halfL && fminf(kx, fminf(ky, kz)) >= 0.0f) {
+        p.x = fmaf(-c.L, kx, p.x); p.y = fmaf(-c.L, ky, p.y); p.z = fmaf(-c.L, kz, p.z);
+        return 1;
+    }
+    return 2;
+}
+
+__device__ __forceinline__ float warp_min_pos(float v)   // v >= 0: integer order == float order
+{
+    return __uint_as_float(__reduce_min_sync(0xffffffffu, __float_as_uint(v)));
+}
+__device__ __forceinline__ float warp_max_pos(float v)
+{
+    return __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(v)));
+}
+
 template <bool GEOM, bool POT, bool COUNT>
 __global__ void __launch_bounds__(GW_THREADS, 2)
 k_walk_group(WalkArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4 *s_tab = reinterpret_cast<float4 *>(smem_raw);
-    WarpSmem *wsm = reinterpret_cast<WarpSmem *>(smem_raw + OG_NTAB * sizeof(float4));
+    WarpSmem *wsm = reinterpret_cast<WarpSmem *>(smem_raw + (OG_NTAB + 1) * sizeof(float4));
     copy_table(s_tab, a.tab);
     __syncthreads();
     const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
     WarpSmem &w = wsm[wid];
     const uint32_t lt = lanemask_lt();
     const uint32_t mybit = 1u << lane;
+    const WalkConst &c = a.c;
     unsigned long long *cnt = COUNT ? a.counters : nullptr;
     uint32_t *sp_start = a.spill + (size_t)(blockIdx.x * GW_WARPS + wid) * 3 * a.spill_cap;
     uint32_t *sp_cnt = sp_start + a.spill_cap, *sp_mask = sp_cnt + a.spill_cap;
 
     for (;;) {
-        uint32_t g = 0;
-        if (lane == 0) g = atomicAdd(a.work, 1u);
-        g = __shfl_sync(0xffffffffu, g, 0);
-        if (g >= a.n_groups) break;
-        const uint32_t k = g * 32u + lane;
+        uint32_t gi = 0;
+        if (lane == 0) gi = atomicAdd(a.work, 1u);
+        gi = __shfl_sync(0xffffffffu, gi, 0);
+        if (gi >= a.n_groups) break;
+        const uint32_t k = gi * 32u + lane;
         const bool valid = k < a.n_active;
+        const uint32_t klast = min(gi * 32u + 31u, a.n_active - 1u);
         uint32_t out = 0;
-        Target t = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0xffffffffu};
-        if (valid) t = load_target(a, k, out, GEOM);
+        // lanes past the end mirror the last target (keeps the group's bounds tight); they never
+        // appear in a mask and write nothing
+        Target t = load_target(a, valid ? k : klast, out, GEOM);
+        t.x = fabsf(t.x); t.y = fabsf(t.y); t.z = fabsf(t.z);   // -0.0 -> +0.0 (integer-ordered reductions below)
+        GroupInfo g;
+        {
+            // positions are >= 0 (0 <= x < L), a_old >= 0, h >= 0
+            const float lox = warp_min_pos(t.x), loy = warp_min_pos(t.y), loz = warp_min_pos(t.z);
+            const float hix = warp_max_pos(t.x), hiy = warp_max_pos(t.y), hiz = warp_max_pos(t.z);
+            g.gcx = 0.5f * (lox + hix); g.gcy = 0.5f * (loy + hiy); g.gcz = 0.5f * (loz + hiz);
+            // half sizes padded by 2 ulp(L) for the rounding of the centre
+            const float pad = 2.4e-7f * c.L;
+            g.ghx = 0.5f * (hix - lox) + pad; g.ghy = 0.5f * (hiy - loy) + pad; g.ghz = 0.5f * (hiz - loz) + pad;
+            g.amin = warp_min_pos(fabsf(t.aold)); g.amax = warp_max_pos(fabsf(t.aold));
+            g.hmax = warp_max_pos(t.h);
+        }
+        const float hi2m = t.h * t.h * (1.0f + OG_GM);   // own softening guard threshold (R16), padded
         Accum acc = {0.f, 0.f, 0.f, 0.f};
         uint32_t c_full = 0, c_cull = 0, c_ain = 0, c_pin = 0, c_psoft = 0, c_pout = 0;
         int top = 0, pl_top = 0;
@@ -234,40 +375,105 @@ k_walk_group(WalkArgs a)
                 uint32_t item, imask;
                 const uint32_t total = pop_items(w.st_start, w.st_cnt, w.st_mask, top, lane, item, imask);
                 uint2 info = make_uint2(0u, 0u);
+                int cls = CL_DROP;
+                float4 sc, aux;
                 if (lane < total) {
                     const NodeRec n = load_node(a, item);
                     info = __ldg(a.info + item);
-                    w.nd_com[lane] = n.com; w.nd_cell[lane] = n.cell;
-                    w.nd_lo[lane] = n.lo; w.nd_hi[lane] = n.hi;
-                    w.bt_mask[lane] = imask;
+                    cls = classify_node<GEOM>(n, g, c, sc, aux);
+                }
+                const uint32_t bA = __ballot_sync(0xffffffffu, cls == CL_ACCEPT);
+                const uint32_t bX = __ballot_sync(0xffffffffu, cls == CL_GENERIC);
+                const uint32_t nA = __popc(bA), nX = __popc(bX);
+                const uint32_t pX = __popc(bX & lt);
+                if (cls == CL_ACCEPT) {
+                    const uint32_t p = __popc(bA & lt);
+                    w.an_com[p] = sc; w.an_mask[p] = imask;
+                } else if (cls == CL_GENERIC) {
+                    w.xn_com[pX] = sc; w.xn_aux[pX] = aux; w.xn_idx[pX] = item;
+                    w.xn_mask[pX] = imask;
                 }
                 __syncwarp();
+                if (COUNT) {   // group-level outcomes counted as the per-target visits they stand for
+                    uint32_t mk = imask;
+                    {
+                        const uint32_t bO = __ballot_sync(0xffffffffu, cls == CL_OPEN);
+                        if (lane == 0) {
+                            atomicAdd(&a.counters[OGC_CL_OPEN], (unsigned long long)__popc(bO));
+                            atomicAdd(&a.counters[OGC_CL_ACCEPT], (unsigned long long)nA);
+                            atomicAdd(&a.counters[OGC_CL_GENERIC], (unsigned long long)nX);
+                            atomicAdd(&a.counters[OGC_CL_DROP], (unsigned long long)(total - nA - nX - __popc(bO)));
+                            atomicAdd(&a.counters[OGC_BATCHES], 1ull);
+                        }
+                    }
+                    for (uint32_t j = 0; j < total; ++j) {
+                        const uint32_t mj = __shfl_sync(0xffffffffu, mk, j);
+                        const int cj = __shfl_sync(0xffffffffu, cls, j);
+                        if ((mj & mybit) && (cj == CL_OPEN || cj == CL_ACCEPT)) ++c_full;
+                        if ((mj & mybit) && cj == CL_DROP) ++c_cull;
+                    }
+                }
+                // class A: every target in the mask accepts; only the cutoff is per lane
+#pragma unroll 2
+                for (uint32_t j = 0; j < nA; ++j) {
+                    if (w.an_mask[j] & mybit) {
+                        const float4 s = w.an_com[j];
+                        const float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
+                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                        if (r2 < c.rcut2_hi) {
+                            bool in = r2 < c.rcut2_lo;
+                            if (!in) in = og_inside_rcut64(s.x, s.y, s.z, t, c, cnt);
+                            if (in) {
+                                og_monopole_core<POT>(s.w, dx, dy, dz, r2, c, s_tab, acc);
+                                if (COUNT) ++c_ain;
+                            }
+                        }
+                    }
+                }
+                // class X: per-lane decision.  Fast test on (s', G M, lhs, near2, cull2); anything within the
+                // band of a threshold, or where a guard could fire, takes the exact out-of-line visit.
                 uint32_t myopen = 0;
-                for (uint32_t j = 0; j < total; ++j) {
+                for (uint32_t j = 0; j < nX; ++j) {
                     bool open = false;
-                    if (w.bt_mask[j] & mybit) {
-                        NodeRec n;
-                        n.com = w.nd_com[j]; n.cell = w.nd_cell[j]; n.lo = w.nd_lo[j]; n.hi = w.nd_hi[j];
-                        if (og_cull(n, t, a.c)) {
+                    if (w.xn_mask[j] & mybit) {
+                        const float4 s = w.xn_com[j];
+                        const float4 x = w.xn_aux[j];
+                        float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
+                        if (x.w != 0.0f) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
+                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                        if (r2 > x.z) {
                             if (COUNT) ++c_cull;
                         } else {
                             if (COUNT) ++c_full;
-                            float dx, dy, dz, r2;
-                            open = og_open<GEOM>(n, t, a.c, dx, dy, dz, r2, cnt);
-                            if (!open) {
-                                const int in = og_monopole<POT>(n, t, a.c, s_tab, dx, dy, dz, r2, acc, cnt);
-                                if (COUNT) c_ain += in;
+                            const float rhs = GEOM ? c.theta2 * r2 : t.A * r2 * r2;
+                            const float diff = x.x - rhs, band = OG_BAND * x.x;
+                            if (diff > band) {
+                                open = true;
+                            } else if (diff < -band && r2 > x.y && r2 > hi2m) {
+                                if (r2 < c.rcut2_hi) {
+                                    bool in = r2 < c.rcut2_lo;
+                                    if (!in) in = og_inside_rcut64(s.x, s.y, s.z, t, c, cnt);
+                                    if (in) {
+                                        og_monopole_core<POT>(s.w, dx, dy, dz, r2, c, s_tab, acc);
+                                        if (COUNT) ++c_ain;
+                                    }
+                                }
+                            } else {
+                                uint32_t n_in = 0;
+                                open = slow_visit<GEOM, POT>(a, w.xn_idx[j], t, s_tab, acc, cnt, n_in);
+                                if (COUNT) c_ain += n_in;
                             }
                         }
                     }
                     const uint32_t b = __ballot_sync(0xffffffffu, open);
-                    if (lane == j) myopen = b;
+                    if (cls == CL_GENERIC && pX == j) myopen = b;
                 }
                 __syncwarp();
                 // push opened internal nodes (children ranges) and opened leaves (particle ranges)
+                const uint32_t cmask = (cls == CL_OPEN) ? imask : myopen;
                 const bool is_leaf = (info.y & OG_LEAF_BIT) != 0;
-                const bool push_n = myopen != 0 && !is_leaf;
-                const bool push_p = myopen != 0 && is_leaf;
+                const bool push_n = cmask != 0 && !is_leaf;
+                const bool push_p = cmask != 0 && is_leaf;
                 const uint32_t bn = __ballot_sync(0xffffffffu, push_n);
                 const uint32_t bp = __ballot_sync(0xffffffffu, push_p);
                 const int nn = __popc(bn);
@@ -297,12 +503,12 @@ k_walk_group(WalkArgs a)
                 }
                 if (push_n) {
                     const int p = top + __popc(bn & lt);
-                    w.st_start[p] = info.x; w.st_cnt[p] = info.y; w.st_mask[p] = myopen;
+                    w.st_start[p] = info.x; w.st_cnt[p] = info.y; w.st_mask[p] = cmask;
                 }
                 top += nn;
                 if (push_p) {
                     const int p = pl_top + __popc(bp & lt);
-                    w.pl_start[p] = info.x; w.pl_cnt[p] = info.y & ~OG_LEAF_BIT; w.pl_mask[p] = myopen;
+                    w.pl_start[p] = info.x; w.pl_cnt[p] = info.y & ~OG_LEAF_BIT; w.pl_mask[p] = cmask;
                 }
                 pl_top += __popc(bp);
                 pl_items += __reduce_add_sync(0xffffffffu, push_p ? (info.y & ~OG_LEAF_BIT) : 0u);
@@ -313,16 +519,48 @@ k_walk_group(WalkArgs a)
                 uint32_t item, imask;
                 const uint32_t total = pop_items(w.pl_start, w.pl_cnt, w.pl_mask, pl_top, lane, item, imask);
                 pl_items -= total;
+                int pc = 0;
+                float4 p;
+                float ph = 0.f;
                 if (lane < total) {
-                    w.pt_pos[lane] = __ldg(a.spos + item);
-                    w.pt_h[lane] = __ldg(a.sh + item);
-                    w.pt_slot[lane] = item;
-                    w.bt_mask[lane] = imask;
+                    p = __ldg(a.spos + item);
+                    ph = __ldg(a.sh + item);
+                    pc = classify_particle(p, g, c);
+                }
+                const uint32_t bs = __ballot_sync(0xffffffffu, pc != 0);
+                const uint32_t ns = __popc(bs);
+                if (pc != 0) {
+                    const uint32_t q = __popc(bs & lt);
+                    w.pt_pos[q] = p; w.pt_h[q] = ph; w.pt_slot[q] = item; w.pt_mask[q] = imask; w.pt_flag[q] = (uint32_t)pc;
                 }
                 __syncwarp();
-                for (uint32_t j = 0; j < total; ++j) {
-                    if ((w.bt_mask[j] & mybit) && w.pt_slot[j] != t.slot) {
-                        const int kind = og_pair<POT>(w.pt_pos[j], w.pt_h[j], t, a.c, s_tab, acc, cnt);
+                if (COUNT) {
+                    const uint32_t b1 = __ballot_sync(0xffffffffu, pc == 1), b2 = __ballot_sync(0xffffffffu, pc == 2);
+                    if (lane == 0) {
+                        atomicAdd(&a.counters[OGC_PT_SHIFT], (unsigned long long)__popc(b1));
+                        atomicAdd(&a.counters[OGC_PT_WRAP], (unsigned long long)__popc(b2));
+                        atomicAdd(&a.counters[OGC_PT_DROP], (unsigned long long)(total - ns));
+                    }
+                    for (uint32_t j = 0; j < total; ++j) {
+                        const uint32_t mj = __shfl_sync(0xffffffffu, imask, j);
+                        const int cj = __shfl_sync(0xffffffffu, pc, j);
+                        const uint32_t sj = __shfl_sync(0xffffffffu, item, j);
+                        if ((mj & mybit) && cj == 0 && sj != t.slot) ++c_pout;
+                    }
+                }
+#pragma unroll 2
+                for (uint32_t j = 0; j < ns; ++j) {
+                    if ((w.pt_mask[j] & mybit) && w.pt_slot[j] != t.slot) {
+                        const float4 q = w.pt_pos[j];
+                        float dx = q.x - t.x, dy = q.y - t.y, dz = q.z - t.z;
+                        if (w.pt_flag[j] == 2u) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
+                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                        int kind = 0;
+                        if (r2 < c.rcut2_hi) {
+                            bool in = r2 < c.rcut2_lo;
+                            if (!in) in = og_inside_rcut64(q.x, q.y, q.z, t, c, cnt);
+                            if (in) kind = og_pair_core<POT>(dx, dy, dz, r2, q.w, w.pt_h[j], t, c, s_tab, acc);
+                        }
                         if (COUNT) { if (kind == 0) ++c_pout; else { ++c_pin; if (kind == 2) ++c_psoft; } }
                     }
                 }
@@ -341,25 +579,27 @@ k_walk_group(WalkArgs a)
             const int slot[6] = {OGC_V_FULL, OGC_V_CULL, OGC_A_IN, OGC_P_IN, OGC_P_SOFT, OGC_P_OUT};
 #pragma unroll
             for (int q = 0; q < 6; ++q) {
-                const uint32_t s = __reduce_add_sync(0xffffffffu, v[q]);
+                const uint32_t s = __reduce_add_sync(0xffffffffu, valid ? v[q] : 0u);
                 if (lane == 0) atomicAdd(&a.counters[slot[q]], (unsigned long long)s);
             }
         }
     }
 }
 
-// split table rows (T, dT, E, dE) in fp64, stored fp32 (R18)
+// split table rows (T, T' dw, E, E' dw) at the nodes w_i = i dw, dw = r_cut / OG_NTAB / (2 r_s), in
+// fp64, stored fp32 (R18).  T' = -(4 w^2 / sqrt(pi)) exp(-w^2), E' = -(2 / sqrt(pi)) exp(-w^2).
 __global__ void k_split_table(float4 *tab, double rcut, double r_s)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= OG_NTAB) return;
+    if (i > OG_NTAB) return;
     const double two_over_sqrt_pi = 1.1283791670955125738961589031215;
-    const double w0 = (double)i * rcut / OG_NTAB / (2.0 * r_s);
-    const double w1 = (double)(i + 1) * rcut / OG_NTAB / (2.0 * r_s);
-    const double T0 = erfc(w0) + two_over_sqrt_pi * w0 * exp(-w0 * w0);
-    const double T1 = erfc(w1) + two_over_sqrt_pi * w1 * exp(-w1 * w1);
-    const double E0 = erfc(w0), E1 = erfc(w1);
-    tab[i] = make_float4((float)T0, (float)(T1 - T0), (float)E0, (float)(E1 - E0));
+    const double dw = rcut / OG_NTAB / (2.0 * r_s);
+    const double w = (double)i * dw;
+    const double ex = exp(-w * w);
+    const double T = erfc(w) + two_over_sqrt_pi * w * ex;
+    const double dT = -2.0 * two_over_sqrt_pi * w * w * ex * dw;
+    const double E = erfc(w), dE = -two_over_sqrt_pi * ex * dw;
+    tab[i] = make_float4((float)T, (float)dT, (float)E, (float)dE);
 }
 
 template <bool GEOM, bool POT, bool COUNT>
@@ -370,7 +610,7 @@ cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
         k_walk_simple<GEOM, POT, COUNT><<<grid, 128, 0, st>>>(a);
         return cudaGetLastError();
     }
-    const size_t smem = OG_NTAB * sizeof(float4) + GW_WARPS * sizeof(WarpSmem);
+    const size_t smem = (OG_NTAB + 1) * sizeof(float4) + GW_WARPS * sizeof(WarpSmem);
     auto kern = k_walk_group<GEOM, POT, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -395,7 +635,7 @@ size_t ogk_walk_spill_bytes(int sm_count)
 
 cudaError_t ogk_split_table(float4 *tab, double rcut, double r_s, cudaStream_t st)
 {
-    k_split_table<<<(OG_NTAB + 255) / 256, 256, 0, st>>>(tab, rcut, r_s);
+    k_split_table<<<(OG_NTAB + 256) / 256, 256, 0, st>>>(tab, rcut, r_s);
     return cudaGetLastError();
 }
 
@@ -420,6 +660,7 @@ cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t 
     c.dG = (double)p.G; c.dalpha = (double)p.alpha; c.dtheta2 = (double)p.theta * (double)p.theta;
     c.L = t->box; c.invL = 1.0f / t->box;
     c.rcut = (float)c.drcut; c.rcut2 = (float)(c.drcut * c.drcut);
+    c.rcut2_lo = c.rcut2 * (1.0f - OG_BAND); c.rcut2_hi = c.rcut2 * (1.0f + OG_BAND);
     c.cull_r = (float)(c.drcut * (1.0 + 1e-5) + 1e-6 * c.dL);
     c.G = p.G; c.alpha = p.alpha; c.theta2 = (float)c.dtheta2;
     c.tab_scale = (float)((double)OG_NTAB / c.drcut);

@@ -11,11 +11,12 @@
 #include "og_internal.cuh"
 
 #define OG_BAND 1.0e-5f
-#define OG_NTAB 1024  // intervals of the split table on [0, r_cut]
+#define OG_NTAB 1024  // intervals of the split table on [0, r_cut]; OG_NTAB + 1 rows
 
 struct WalkConst {
     float L, invL;
     float rcut, rcut2;
+    float rcut2_lo, rcut2_hi;   // rcut2 * (1 -+ OG_BAND): outside this band the fp32 cutoff test is final
     float cull_r;        // r_cut * (1 + 1e-5) + 1e-6 L : conservative cull radius
     float G;
     float alpha;
@@ -44,15 +45,18 @@ __device__ __forceinline__ float og_wrap(float d, const WalkConst &c)
 
 __device__ __forceinline__ double og_wrap64(double d, double L) { return d - L * round(d / L); }
 
-// (T, dT, E, dE) rows in shared memory: T(w) = erfc(w) + 2w/sqrt(pi) exp(-w^2), E = erfc(w),
-// w = r / (2 r_s), tabulated on r in [0, r_cut] and linearly interpolated (R18).
+// (T, T', E, E') rows in shared memory: T(w) = erfc(w) + 2w/sqrt(pi) exp(-w^2), E = erfc(w),
+// w = r / (2 r_s), tabulated at the OG_NTAB + 1 nodes t = r * OG_NTAB / r_cut = 0..OG_NTAB with the
+// derivative per table step; evaluated as value + (t - nearest node) * derivative (R18; error
+// <= step^2/8 max|T''| ~ 8e-7).  The nearest node comes from the float rounding of t + 1.5 * 2^23
+// (no F2I / I2F in the hot loop).
 __device__ __forceinline__ void og_split(const float4 *__restrict__ tab, float r, const WalkConst &c,
                                          float &T, float &E)
 {
-    const float t = r * c.tab_scale;
-    int i = (int)t;
-    i = min(i, OG_NTAB - 1);
-    const float f = t - (float)i;
+    const float MAGIC = 12582912.0f;
+    const float tf = fmaf(r, c.tab_scale, MAGIC);
+    const int i = min(__float_as_int(tf) & 0x7ff, OG_NTAB);
+    const float f = fmaf(r, c.tab_scale, MAGIC - tf);
     const float4 row = tab[i];
     T = fmaf(f, row.y, row.x);
     E = fmaf(f, row.w, row.z);
@@ -73,22 +77,19 @@ __device__ __noinline__ bool og_inside_rcut64(float sx, float sy, float sz, cons
 __device__ __forceinline__ bool og_inside_rcut(float r2, float sx, float sy, float sz, const Target &t,
                                                const WalkConst &c, unsigned long long *counters)
 {
-    bool in = r2 < c.rcut2;
-    if (fabsf(r2 - c.rcut2) <= OG_BAND * c.rcut2) in = og_inside_rcut64(sx, sy, sz, t, c, counters);
+    bool in = r2 < c.rcut2_lo;
+    if (!in && r2 < c.rcut2_hi) in = og_inside_rcut64(sx, sy, sz, t, c, counters);
     return in;
 }
 
 // ---- pair kernel C5 ------------------------------------------------------------------------
-// Source particle (px, py, pz, pm, ph); adds to acc if r < r_cut.  Returns 0 outside, 1 inside
-// with r >= h, 2 inside with r < h.
+// Interaction with a source particle at nearest-image offset d (|d|^2 = r2, already known to be
+// inside r_cut), mass pm, softening length ph.  Returns 1 for r >= h, 2 for r < h.
 template <bool POT>
-__device__ __forceinline__ int og_pair(const float4 p, float ph, const Target &t, const WalkConst &c,
-                                       const float4 *__restrict__ tab, Accum &acc,
-                                       unsigned long long *counters)
+__device__ __forceinline__ int og_pair_core(float dx, float dy, float dz, float r2, float pm, float ph,
+                                            const Target &t, const WalkConst &c,
+                                            const float4 *__restrict__ tab, Accum &acc)
 {
-    const float dx = og_wrap(p.x - t.x, c), dy = og_wrap(p.y - t.y, c), dz = og_wrap(p.z - t.z, c);
-    float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    if (!og_inside_rcut(r2, p.x, p.y, p.z, t, c, counters)) return 0;
     r2 = fmaxf(r2, 1.0e-36f);           // distinct coincident particles: force 0, potential -14/5 m/h
     const float rinv = rsqrtf(r2);
     const float r = r2 * rinv;
@@ -118,13 +119,26 @@ __device__ __forceinline__ int og_pair(const float4 p, float ph, const Target &t
                          0.06666666666666667f * uinv);
         }
     }
-    const float gm = c.G * p.w;
+    const float gm = c.G * pm;
     const float f = gm * g * T;
     acc.ax = fmaf(f, dx, acc.ax);
     acc.ay = fmaf(f, dy, acc.ay);
     acc.az = fmaf(f, dz, acc.az);
     if (POT) acc.pot = fmaf(gm * pp, E, acc.pot);
     return kind;
+}
+
+// Source particle p = (x, y, z, m) in any periodic image; adds to acc if r < r_cut.  Returns 0
+// outside, 1 inside with r >= h, 2 inside with r < h.
+template <bool POT>
+__device__ __forceinline__ int og_pair(const float4 p, float ph, const Target &t, const WalkConst &c,
+                                       const float4 *__restrict__ tab, Accum &acc,
+                                       unsigned long long *counters)
+{
+    const float dx = og_wrap(p.x - t.x, c), dy = og_wrap(p.y - t.y, c), dz = og_wrap(p.z - t.z, c);
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    if (!og_inside_rcut(r2, p.x, p.y, p.z, t, c, counters)) return 0;
+    return og_pair_core<POT>(dx, dy, dz, r2, p.w, ph, t, c, tab, acc);
 }
 
 // ---- node: cull, opening decision, monopole ------------------------------------------------
@@ -216,6 +230,24 @@ __device__ __forceinline__ bool og_open(const NodeRec &n, const Target &t, const
     return open;
 }
 
+// Monopole of mass GM = G * M at offset d (r2 inside r_cut), Newtonian force times the split
+// factor (R21).
+template <bool POT>
+__device__ __forceinline__ void og_monopole_core(float GM, float dx, float dy, float dz, float r2,
+                                                 const WalkConst &c, const float4 *__restrict__ tab, Accum &acc)
+{
+    const float rinv = rsqrtf(r2);
+    const float r = r2 * rinv;
+    float T, E;
+    og_split(tab, r, c, T, E);
+    const float gr = GM * rinv;
+    const float f = gr * T * (rinv * rinv);
+    acc.ax = fmaf(f, dx, acc.ax);
+    acc.ay = fmaf(f, dy, acc.ay);
+    acc.az = fmaf(f, dz, acc.az);
+    if (POT) acc.pot = fmaf(-gr, E, acc.pot);
+}
+
 // C6 step 4: accepted node, Newtonian monopole times the split factor (R21).  Returns 1 if
 // r < r_cut.
 template <bool POT>
@@ -224,15 +256,6 @@ __device__ __forceinline__ int og_monopole(const NodeRec &n, const Target &t, co
                                            float r2, Accum &acc, unsigned long long *counters)
 {
     if (!og_inside_rcut(r2, n.com.x, n.com.y, n.com.z, t, c, counters)) return 0;
-    const float rinv = rsqrtf(r2);
-    const float r = r2 * rinv;
-    float T, E;
-    og_split(tab, r, c, T, E);
-    const float gm = c.G * n.com.w;
-    const float f = gm * T * rinv * rinv * rinv;
-    acc.ax = fmaf(f, dx, acc.ax);
-    acc.ay = fmaf(f, dy, acc.ay);
-    acc.az = fmaf(f, dz, acc.az);
-    if (POT) acc.pot = fmaf(-gm * rinv, E, acc.pot);
+    og_monopole_core<POT>(c.G * n.com.w, dx, dy, dz, r2, c, tab, acc);
     return 1;
 }
