@@ -25,7 +25,7 @@ inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct Layout {
     size_t keysA, keysB, idxA, idxB, sort_scratch, spos, sh, inv_perm;
-    size_t level, first, count, first_child, nchild, com, cell, lo, hi, info;
+    size_t level, first, count, first_child, nchild, com, cell, lo, hi, info, n1, n2;
     size_t oct_scratch, level_start, status, counters, split_tab, spill, total;
 };
 
@@ -43,6 +43,7 @@ Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count)
     L.nchild = take(M);
     L.com = take(M * 16); L.cell = take(M * 16); L.lo = take(M * 16); L.hi = take(M * 16);
     L.info = take(M * 8);
+    L.n1 = take(M * 16); L.n2 = take(M * 16);
     L.oct_scratch = take(ogk_octree_scratch_bytes(max_nodes));
     L.level_start = take(24 * 4);
     L.status = take(16 * 4);
@@ -175,6 +176,7 @@ extern "C" og_tree *og_tree_build(const float *pos, const float *mass, const flo
     t->node_nchild = (uint8_t *)(b + L.nchild);
     t->node_com = (float4 *)(b + L.com); t->node_cell = (float4 *)(b + L.cell);
     t->node_lo = (float4 *)(b + L.lo); t->node_hi = (float4 *)(b + L.hi); t->node_info = (uint2 *)(b + L.info);
+    t->node_n1 = (uint4 *)(b + L.n1); t->node_n2 = (float4 *)(b + L.n2);
     t->d_level_start = (uint32_t *)(b + L.level_start); t->d_status = (uint32_t *)(b + L.status);
     t->d_counters = (unsigned long long *)(b + L.counters);
     t->split_tab = (float4 *)(b + L.split_tab);

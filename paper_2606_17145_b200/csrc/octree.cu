@@ -211,6 +211,9 @@ struct UpArgs {
     double4 *sums;      // (M, sum m x, sum m y, sum m z) per node, fp64
     float4 *com, *cell, *lo, *hi;
     uint2 *info;
+    uint4 *n1;
+    float4 *n2;
+    uint32_t *status;
 };
 
 __device__ __forceinline__ uint32_t og_compact3(uint64_t x)
@@ -305,6 +308,27 @@ k_upward(UpArgs a)
             up_store(a, j, M, ax, ay, az, lo, hi, hm);
         }
     }
+    // (C) packed walk records n1, n2 (og_internal.cuh) from the finished fp32 records.  R and ng are
+    // bounds used only by conservative tests of the walk, so they are rounded up.
+    grid.sync();
+    for (uint32_t j = t0; j < n_nodes; j += stride) {
+        const float4 s = __ldcg(a.com + j), cc = __ldcg(a.cell + j), lo = __ldcg(a.lo + j), hi = __ldcg(a.hi + j);
+        const uint2 info = __ldcg(a.info + j);
+        const double ex = fmax((double)s.x - (double)lo.x, (double)hi.x - (double)s.x),
+                     ey = fmax((double)s.y - (double)lo.y, (double)hi.y - (double)s.y),
+                     ez = fmax((double)s.z - (double)lo.z, (double)hi.z - (double)s.z);
+        const float R = __double2float_ru(sqrt(ex * ex + ey * ey + ez * ez) * (1.0 + 1e-6));
+        const double lim = 0.6 * (double)cc.w;
+        const double gx = lim + fabs((double)s.x - (double)cc.x), gy = lim + fabs((double)s.y - (double)cc.y),
+                     gz = lim + fabs((double)s.z - (double)cc.z);
+        const float rg = __double2float_ru(sqrt(gx * gx + gy * gy + gz * gz) * (1.0 + 1e-6));
+        const uint32_t leaf = (info.y & OG_LEAF_BIT) ? 1u : 0u;
+        const uint32_t cnt = info.y & ~OG_LEAF_BIT;
+        if (cnt >= (1u << 26)) atomicOr(a.status, OG_DEV_NODE_OVERFLOW);   // does not fit the packed record
+        const uint32_t meta = ((uint32_t)a.level[j] << 27) | (leaf << 26) | (cnt & 0x03ffffffu);
+        a.n1[j] = make_uint4(__float_as_uint(R), __float_as_uint(fmaxf(rg, lo.w)), info.x, meta);
+        a.n2[j] = make_float4(cc.x, cc.y, cc.z, lo.w);
+    }
 }
 
 int coop_grid(const void *kernel, int threads, int sm_count)
@@ -340,7 +364,7 @@ cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st)
     if (e != cudaSuccess) return e;
     UpArgs ua{t->keys, t->spos, t->sh, t->box, t->node_level, t->node_first, t->node_count,
               t->node_first_child, t->node_nchild, t->d_level_start, sums, t->node_com, t->node_cell,
-              t->node_lo, t->node_hi, t->node_info};
+              t->node_lo, t->node_hi, t->node_info, t->node_n1, t->node_n2, t->d_status};
     void *args2[] = {&ua};
     e = cudaLaunchCooperativeKernel((const void *)k_upward,
                                     dim3(coop_grid((const void *)k_upward, OCT_THREADS, t->sm_count)),

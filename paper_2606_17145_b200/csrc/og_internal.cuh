@@ -58,6 +58,14 @@ struct og_tree {
     float4 *node_lo;
     float4 *node_hi;
     uint2 *node_info;
+    // packed walk records (read by the group walk; written by the last phase of k_upward):
+    //   n0 = node_com
+    //   n1 = (R, ng, first, meta): R = largest distance from s to a corner of the AABB (rounded up),
+    //        ng = max(h_max, largest |x - s| over the 0.6 l guard box of R15) (rounded up), first = first
+    //        child / first slot, meta = level << 27 | leaf << 26 | (n_child or particle count)
+    //   n2 = (c_x, c_y, c_z, h_max)
+    uint4 *node_n1;
+    float4 *node_n2;
     float4 *split_tab;         // OG_NTAB rows (T, dT, E, dE), see walk_math.cuh
     // small device state
     uint32_t *d_level_start;   // [24]: start index per level, [22] = n_nodes, [23] = max level

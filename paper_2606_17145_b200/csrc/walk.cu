@@ -23,8 +23,10 @@
 namespace {
 
 struct WalkArgs {
-    const float4 *com, *cell, *lo, *hi;
+    const float4 *com, *cell, *lo, *hi;   // full node records (exact path, simple walk); com doubles as n0
     const uint2 *info;
+    const uint4 *n1;           // packed walk record (R, ng, first, meta), og_internal.cuh
+    const float4 *n2;          // (c_x, c_y, c_z, h_max)
     const float4 *spos;
     const float *sh;
     const float4 *tab;
@@ -75,7 +77,7 @@ __device__ __forceinline__ void copy_table(float4 *s_tab, const float4 *g_tab)
 // -------------------------------------------------------------------------------------------
 template <bool GEOM, bool POT, bool COUNT>
 __global__ void __launch_bounds__(128)
-k_walk_simple(WalkArgs a)
+k_walk_simple(const __grid_constant__ WalkArgs a)
 {
     __shared__ float4 s_tab[OG_NTAB + 1];
     copy_table(s_tab, a.tab);
@@ -135,17 +137,23 @@ constexpr int GW_THREADS = GW_WARPS * 32;
 constexpr int GW_STACK = 256;         // node-range stack entries per warp in shared memory
 constexpr int GW_SPILL = 128;         // entries moved to / from global memory at a time
 constexpr int GW_PLIST = 64;          // particle-range list entries per warp
+constexpr int GW_NSEG = 8;            // 32-source segments buffered per warp before they are evaluated
 
+#define SEG_WRAP 1u      // some source of the segment is not pre-shifted: per-lane nearest-image wrap
+#define SEG_PART 2u      // particle segment (else node segment); only the counters care
+
+// Per-warp working set.  Sources (accepted nodes and particles of opened leaves) are
+// buffered in `ring_*` in segments of 32 slots; W[seg][lane] has bit j set iff lane's target interacts
+// with slot j of the segment.  Each lane later walks its OWN set bits (per-lane compaction), so a lane
+// is idle only when its list is shorter than the longest one of the buffered window.
 struct __align__(16) WarpSmem {
-    float4 xn_com[32], xn_aux[32];                          // class X (per-lane decision): (s', GM), (lhs, near2, cull2, wrap)
+    float4 ring_pos[GW_NSEG * 32];      // (x', y', z', G m): pre-shifted to the group's periodic image
+    float ring_h[GW_NSEG * 32];         // softening length of the source (0 for nodes)
+    uint32_t W[GW_NSEG][32];
+    float4 xn_com[32], xn_aux[32], xn_cel[32];   // undecided nodes: (s', GM), (lhs, near2, cull2, band), (c', l)
+    float xn_hm2[32];                   // h_max^2
     uint32_t xn_idx[32];
-    float4 an_com[32];                                      // class A (accepted by all) nodes: (s', GM)
-    float4 pt_pos[32];                                      // staged particles (x', y', z', m)
-    float pt_h[32];
-    uint32_t pt_slot[32];
-    uint32_t pt_mask[32];             // bit 31.. : lane masks; pt_flag: generic (per-lane wrap) or shifted
-    uint32_t pt_flag[32];
-    uint32_t xn_mask[32], an_mask[32];
+    uint32_t seg_flags[GW_NSEG];
     uint32_t st_start[GW_STACK], st_cnt[GW_STACK], st_mask[GW_STACK];
     uint32_t pl_start[GW_PLIST], pl_cnt[GW_PLIST], pl_mask[GW_PLIST];
 };
@@ -155,6 +163,20 @@ __device__ __forceinline__ uint32_t lanemask_lt()
     uint32_t m;
     asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
     return m;
+}
+
+// 32 x 32 bit-matrix transpose across the warp: lane j passes row j (bit t = element (j, t)); lane t
+// receives column t (bit j = element (j, t)).  Five butterfly stages.
+__device__ __forceinline__ uint32_t transpose32(uint32_t x, uint32_t lane)
+{
+#pragma unroll
+    for (int k = 16; k >= 1; k >>= 1) {
+        const uint32_t m = (k == 16) ? 0x0000ffffu : (k == 8) ? 0x00ff00ffu : (k == 4) ? 0x0f0f0f0fu
+                         : (k == 2) ? 0x33333333u : 0x55555555u;
+        const uint32_t y = __shfl_xor_sync(0xffffffffu, x, k);
+        x = (lane & k) ? (((y >> k) & m) | (x & ~m)) : ((x & m) | ((y << k) & ~m));
+    }
+    return x;
 }
 
 // Pops up to 32 items from the top of a range list.  Lane j < total receives item index and
@@ -192,42 +214,42 @@ __device__ __forceinline__ uint32_t pop_items(uint32_t *s_start, uint32_t *s_cnt
 // of a_old, largest softening length.
 struct GroupInfo {
     float gcx, gcy, gcz, ghx, ghy, ghz;
-    float amin, amax, hmax;
+    float amin, amax, hmax2;
 };
 
 enum { CL_DROP = 0, CL_OPEN = 1, CL_ACCEPT = 2, CL_GENERIC = 3 };
 
 #define OG_GM 1.0e-4f   // relative safety margin of the group-level (conservative) classifications
 
-// Group-level classification of one node by the lane that loaded it.  Every
-// outcome other than CL_GENERIC is one that EVERY target of the group would reach on its own:
-//   CL_DROP    no target can be within r_cut of the node's AABB (cutoff-box test, result-neutral), or
-//              all accept it but none is within r_cut of its centre of mass;
-//   CL_OPEN    every target opens it (relative / geometric criterion at the largest possible r and
-//              a_old, or the group lies inside the 0.6 l guard box, or inside the softening guard);
-//   CL_ACCEPT  every target accepts it (criterion at the smallest possible r and a_old, no guard can
-//              fire) and one exact periodic shift serves all targets: `sc` = (s - k L, G M).
+// Group-level classification of one node by the lane that loaded it, from the packed
+// walk record n0 = (s, M), n1 = (R, ng, first, meta): R = largest distance from s to a corner of the
+// node's AABB, ng = max(h_max, largest |x - s| of a point inside the 0.6 l guard box).  Every outcome
+// other than CL_GENERIC is one that EVERY target of the group would reach on its own:
+//   CL_DROP    no target is within r_cut + R of s (then no particle of the node is within r_cut of any
+//              target and r_COM > r_cut: the node contributes nothing whether accepted or opened, R17),
+//              or all accept it but none is within r_cut of s;
+//   CL_OPEN    every target opens it by the relative / geometric criterion (largest possible r, a_old);
+//   CL_ACCEPT  every target accepts it (criterion at the smallest possible r and a_old, and no target
+//              is within ng or its own h of s, so no guard can fire).
+// `sc` = (s - k L, G M): one exact periodic shift serves all targets if `shifted` (k = 0, or k = +1 with
+// s >= L/2), else sc holds s itself and the lanes wrap.
 template <bool GEOM>
-__device__ __forceinline__ int classify_node(const NodeRec &n, const GroupInfo &g, const WalkConst &c, float4 &sc,
-                                             float4 &aux)
+__device__ __forceinline__ int classify_node(const float4 n0, float R, float ng, float l, const GroupInfo &g,
+                                             const WalkConst &c, float4 &sc, float4 &aux, bool &shifted,
+                                             float &kx, float &ky, float &kz)
 {
-    const float l = n.cell.w;
-    // cutoff box against the group's bounding box
-    const float gapx = fabsf(og_wrap(0.5f * (n.lo.x + n.hi.x) - g.gcx, c)) - 0.5f * (n.hi.x - n.lo.x) - g.ghx;
-    const float gapy = fabsf(og_wrap(0.5f * (n.lo.y + n.hi.y) - g.gcy, c)) - 0.5f * (n.hi.y - n.lo.y) - g.ghy;
-    const float gapz = fabsf(og_wrap(0.5f * (n.lo.z + n.hi.z) - g.gcz, c)) - 0.5f * (n.hi.z - n.lo.z) - g.ghz;
-    if (fmaxf(gapx, fmaxf(gapy, gapz)) > c.cull_r) return CL_DROP;
-    // distance range |s - x| over the group's box, per axis (valid on the periodic circle)
-    const float kx = rintf((n.com.x - g.gcx) * c.invL), ky = rintf((n.com.y - g.gcy) * c.invL),
-                kz = rintf((n.com.z - g.gcz) * c.invL);
-    const float adx = fabsf(fmaf(-c.L, kx, n.com.x - g.gcx)), ady = fabsf(fmaf(-c.L, ky, n.com.y - g.gcy)),
-                adz = fabsf(fmaf(-c.L, kz, n.com.z - g.gcz));
+    kx = rintf((n0.x - g.gcx) * c.invL); ky = rintf((n0.y - g.gcy) * c.invL); kz = rintf((n0.z - g.gcz) * c.invL);
+    const float adx = fabsf(fmaf(-c.L, kx, n0.x - g.gcx)), ady = fabsf(fmaf(-c.L, ky, n0.y - g.gcy)),
+                adz = fabsf(fmaf(-c.L, kz, n0.z - g.gcz));
     const float nx = fmaxf(adx - g.ghx, 0.f), ny = fmaxf(ady - g.ghy, 0.f), nz = fmaxf(adz - g.ghz, 0.f);
     const float fx = adx + g.ghx, fy = ady + g.ghy, fz = adz + g.ghz;
     const float rmin2 = fmaf(nz, nz, fmaf(ny, ny, nx * nx));
     const float rmax2 = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
+    const float rc = c.cull_r + R;
+    const float cull2 = rc * rc;
+    if (rmin2 > cull2) return CL_DROP;
     const float l2 = l * l;
-    const float GM = c.G * n.com.w;
+    const float GM = c.G * n0.w;
     float lhs, rhs_max, rhs_min;
     if (GEOM) {
         lhs = l2; rhs_max = c.theta2 * rmax2; rhs_min = c.theta2 * rmin2;
@@ -237,46 +259,27 @@ __device__ __forceinline__ int classify_node(const NodeRec &n, const GroupInfo &
         rhs_min = c.alpha * g.amin * rmin2 * rmin2;
     }
     if (lhs > rhs_max * (1.0f + OG_GM)) return CL_OPEN;
-    // inside guard R15 at group level: offsets of the group's box from the cell centre, per axis
-    const float icx = fabsf(og_wrap(n.cell.x - g.gcx, c)), icy = fabsf(og_wrap(n.cell.y - g.gcy, c)),
-                icz = fabsf(og_wrap(n.cell.z - g.gcz, c));
-    if (fmaxf(icx + g.ghx, fmaxf(icy + g.ghy, icz + g.ghz)) < 0.6f * l * (1.0f - OG_GM)) return CL_OPEN;   // all inside
-    if (rmax2 < n.lo.w * n.lo.w * (1.0f - OG_GM)) return CL_OPEN;                       // R16 fires for all
-    // no target can be inside the guard box if the group's box misses it on some axis
-    const bool no_inside = fmaxf(icx - g.ghx, fmaxf(icy - g.ghy, icz - g.ghz)) > 0.6f * l * (1.0f + OG_GM);
-    const float hh = fmaxf(g.hmax, n.lo.w);
-    const bool no_guard = no_inside && rmin2 > hh * hh * (1.0f + OG_GM);
-    // one periodic image for all targets, and s - k L exact (k = 0, or k = +1 with s >= L/2)
-    const bool shifted = fmaxf(fx, fmaxf(fy, fz)) < 0.5f * c.L * (1.0f - OG_GM) && fminf(kx, fminf(ky, kz)) >= 0.0f;
-    if (shifted) sc = make_float4(fmaf(-c.L, kx, n.com.x), fmaf(-c.L, ky, n.com.y), fmaf(-c.L, kz, n.com.z), GM);
-    else sc = make_float4(n.com.x, n.com.y, n.com.z, GM);
-    if (no_guard && lhs < rhs_min * (1.0f - OG_GM)) {
+    shifted = fmaxf(fx, fmaxf(fy, fz)) < 0.5f * c.L * (1.0f - OG_GM) && fminf(kx, fminf(ky, kz)) >= 0.0f;
+    if (shifted) sc = make_float4(fmaf(-c.L, kx, n0.x), fmaf(-c.L, ky, n0.y), fmaf(-c.L, kz, n0.z), GM);
+    else sc = make_float4(n0.x, n0.y, n0.z, GM);
+    const float ng2 = ng * ng;
+    if (lhs < rhs_min * (1.0f - OG_GM) && rmin2 > fmaxf(ng2, g.hmax2) * (1.0f + OG_GM)) {
         if (rmin2 > c.rcut2 * (1.0f + OG_GM)) return CL_DROP;
-        if (shifted) return CL_ACCEPT;
+        return CL_ACCEPT;
     }
-    // undecided: what the per-lane fast test needs.  near2 = below this r^2 a guard could fire and the exact
-    // test is taken; cull2 = (r_cut + R)^2 with R = largest distance from s to a corner of the AABB.
-    const float ex = fmaxf(n.com.x - n.lo.x, n.hi.x - n.com.x), ey = fmaxf(n.com.y - n.lo.y, n.hi.y - n.com.y),
-                ez = fmaxf(n.com.z - n.lo.z, n.hi.z - n.com.z);
-    const float R = sqrtf(fmaf(ez, ez, fmaf(ey, ey, ex * ex))) * (1.0f + OG_GM);
-    const float rc = c.cull_r + R;
-    const float near2 = fmaxf(no_inside ? 0.0f : 3.7f * l2, n.lo.w * n.lo.w * (1.0f + OG_GM));
-    aux = make_float4(lhs, near2, rc * rc, shifted ? 0.0f : 1.0f);
+    aux = make_float4(lhs, ng2 * (1.0f + OG_GM), cull2, OG_BAND * lhs);
     return CL_GENERIC;
 }
 
-// Exact per-lane visit of one node from its full record (cull, opening test with fp64 band, monopole).
-// Out of line: taken only by the few (lane, node) pairs the fast test cannot settle.
-template <bool GEOM, bool POT>
-__device__ __noinline__ bool slow_visit(const WalkArgs &a, uint32_t node, const Target &t, const float4 *s_tab,
-                                        Accum &acc, unsigned long long *cnt, uint32_t &n_in)
+// Exact per-lane decision for one node from its full record (AABB cull, opening test with fp64 band):
+// 0 = culled, 1 = open, 2 = accept.  Out of line: taken only when an fp32 test is within its band.
+template <bool GEOM>
+__device__ __noinline__ int slow_decide(const WalkArgs &a, uint32_t node, const Target &t, unsigned long long *cnt)
 {
     const NodeRec m = load_node(a, node);
-    if (og_cull(m, t, a.c)) return false;
+    if (og_cull(m, t, a.c)) return 0;
     float dx, dy, dz, r2;
-    if (og_open<GEOM>(m, t, a.c, dx, dy, dz, r2, cnt)) return true;
-    n_in += og_monopole<POT>(m, t, a.c, s_tab, dx, dy, dz, r2, acc, cnt);
-    return false;
+    return og_open<GEOM>(m, t, a.c, dx, dy, dz, r2, cnt) ? 1 : 2;
 }
 
 // Group-level treatment of one particle by the lane that loaded it: 0 = no target within r_cut
@@ -305,9 +308,51 @@ __device__ __forceinline__ float warp_max_pos(float v)
     return __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(v)));
 }
 
+// Evaluates the buffered segments: every lane walks the set bits of its own words W[seg][lane] and adds
+// the pair kernel C5 for each (nodes are sources with h = 0: the softening guard R16 guarantees r >= h_i).
+template <bool POT, bool COUNT>
+__device__ __forceinline__ void consume(WarpSmem &w, int nseg, const Target &t, const WalkConst &c,
+                                        const float4 *__restrict__ s_tab, Accum &acc, uint32_t lane,
+                                        unsigned long long *cnt, uint32_t &c_ain, uint32_t &c_pin,
+                                        uint32_t &c_psoft, uint32_t &c_pout)
+{
+    int seg = 0;
+    uint32_t cur = w.W[0][lane];
+    uint32_t fl = w.seg_flags[0];
+    for (;;) {
+        while (cur == 0u && seg + 1 < nseg) {
+            ++seg;
+            cur = w.W[seg][lane];
+            fl = w.seg_flags[seg];
+        }
+        if (!__any_sync(0xffffffffu, cur != 0u)) break;
+        if (cur != 0u) {
+            const int j = __ffs(cur) - 1;
+            cur &= cur - 1u;
+            const int e = seg * 32 + j;
+            const float4 q = w.ring_pos[e];
+            const float hj = w.ring_h[e];
+            float dx = q.x - t.x, dy = q.y - t.y, dz = q.z - t.z;
+            if (fl & SEG_WRAP) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            int kind = 0;
+            if (r2 < c.rcut2_hi) {
+                bool in = r2 < c.rcut2_lo;
+                if (!in) in = og_inside_rcut64(q.x, q.y, q.z, t, c, cnt);
+                if (in) kind = og_pair_core<POT>(dx, dy, dz, r2, q.w, hj, t, c, s_tab, acc);
+            }
+            if (COUNT) {
+                if (fl & SEG_PART) { if (kind == 0) ++c_pout; else { ++c_pin; if (kind == 2) ++c_psoft; } }
+                else if (kind != 0) ++c_ain;
+            }
+        }
+    }
+    __syncwarp();
+}
+
 template <bool GEOM, bool POT, bool COUNT>
 __global__ void __launch_bounds__(GW_THREADS, 2)
-k_walk_group(WalkArgs a)
+k_walk_group(const __grid_constant__ WalkArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4 *s_tab = reinterpret_cast<float4 *>(smem_raw);
@@ -346,12 +391,16 @@ k_walk_group(WalkArgs a)
             const float pad = 2.4e-7f * c.L;
             g.ghx = 0.5f * (hix - lox) + pad; g.ghy = 0.5f * (hiy - loy) + pad; g.ghz = 0.5f * (hiz - loz) + pad;
             g.amin = warp_min_pos(fabsf(t.aold)); g.amax = warp_max_pos(fabsf(t.aold));
-            g.hmax = warp_max_pos(t.h);
+            const float hm = warp_max_pos(t.h);
+            g.hmax2 = hm * hm;
         }
-        const float hi2m = t.h * t.h * (1.0f + OG_GM);   // own softening guard threshold (R16), padded
+        // lanes whose target is the same sorted slot (duplicates in active_idx; the mirrored tail lanes)
+        const uint32_t peers = __match_any_sync(0xffffffffu, t.slot);
+        const float hi2 = t.h * t.h;
+        const float hi2m = hi2 * (1.0f + OG_GM);   // own softening guard threshold (R16), padded
         Accum acc = {0.f, 0.f, 0.f, 0.f};
         uint32_t c_full = 0, c_cull = 0, c_ain = 0, c_pin = 0, c_psoft = 0, c_pout = 0;
-        int top = 0, pl_top = 0;
+        int top = 0, pl_top = 0, nseg = 0;
         uint32_t pl_items = 0, spill_n = 0;
         {
             const uint32_t vm = __ballot_sync(0xffffffffu, valid);
@@ -372,106 +421,126 @@ k_walk_group(WalkArgs a)
                 __syncwarp();
             }
             if (top > 0) {
+                if (nseg == GW_NSEG) {
+                    consume<POT, COUNT>(w, nseg, t, c, s_tab, acc, lane, cnt, c_ain, c_pin, c_psoft, c_pout);
+                    nseg = 0;
+                }
                 uint32_t item, imask;
                 const uint32_t total = pop_items(w.st_start, w.st_cnt, w.st_mask, top, lane, item, imask);
-                uint2 info = make_uint2(0u, 0u);
+                uint32_t first = 0, meta = 0;
                 int cls = CL_DROP;
-                float4 sc, aux;
+                bool shifted = true;
                 if (lane < total) {
-                    const NodeRec n = load_node(a, item);
-                    info = __ldg(a.info + item);
-                    cls = classify_node<GEOM>(n, g, c, sc, aux);
+                    const float4 n0 = __ldg(a.com + item);
+                    const uint4 n1 = __ldg(a.n1 + item);
+                    const float4 n2 = __ldg(a.n2 + item);
+                    first = n1.z; meta = n1.w;
+                    const float l = c.L * __uint_as_float((127u - (meta >> 27)) << 23);   // L / 2^level, exact
+                    float4 sc, aux;
+                    float kx, ky, kz;
+                    cls = classify_node<GEOM>(n0, __uint_as_float(n1.x), __uint_as_float(n1.y), l, g, c, sc, aux,
+                                              shifted, kx, ky, kz);
+                    if (cls >= CL_ACCEPT) {
+                        w.ring_pos[nseg * 32 + lane] = sc;
+                        w.ring_h[nseg * 32 + lane] = 0.0f;
+                    }
+                    if (cls == CL_GENERIC) {
+                        w.xn_com[lane] = sc; w.xn_aux[lane] = aux;
+                        // cell centre in the same periodic image as sc (exact for k in {0, 1}, see classify_node)
+                        w.xn_cel[lane] = shifted ? make_float4(fmaf(-c.L, kx, n2.x), fmaf(-c.L, ky, n2.y),
+                                                               fmaf(-c.L, kz, n2.z), l)
+                                                 : make_float4(n2.x, n2.y, n2.z, l);
+                        w.xn_hm2[lane] = n2.w * n2.w;
+                        w.xn_idx[lane] = item;
+                    }
                 }
                 const uint32_t bA = __ballot_sync(0xffffffffu, cls == CL_ACCEPT);
                 const uint32_t bX = __ballot_sync(0xffffffffu, cls == CL_GENERIC);
-                const uint32_t nA = __popc(bA), nX = __popc(bX);
-                const uint32_t pX = __popc(bX & lt);
-                if (cls == CL_ACCEPT) {
-                    const uint32_t p = __popc(bA & lt);
-                    w.an_com[p] = sc; w.an_mask[p] = imask;
-                } else if (cls == CL_GENERIC) {
-                    w.xn_com[pX] = sc; w.xn_aux[pX] = aux; w.xn_idx[pX] = item;
-                    w.xn_mask[pX] = imask;
-                }
+                const uint32_t bW = __ballot_sync(0xffffffffu, cls >= CL_ACCEPT && !shifted);
+                // Mt: bit j = my target is in the mask of the node lane j holds
+                const uint32_t Mt = transpose32((cls >= CL_ACCEPT) ? imask : 0u, lane);
                 __syncwarp();
                 if (COUNT) {   // group-level outcomes counted as the per-target visits they stand for
-                    uint32_t mk = imask;
-                    {
-                        const uint32_t bO = __ballot_sync(0xffffffffu, cls == CL_OPEN);
-                        if (lane == 0) {
-                            atomicAdd(&a.counters[OGC_CL_OPEN], (unsigned long long)__popc(bO));
-                            atomicAdd(&a.counters[OGC_CL_ACCEPT], (unsigned long long)nA);
-                            atomicAdd(&a.counters[OGC_CL_GENERIC], (unsigned long long)nX);
-                            atomicAdd(&a.counters[OGC_CL_DROP], (unsigned long long)(total - nA - nX - __popc(bO)));
-                            atomicAdd(&a.counters[OGC_BATCHES], 1ull);
-                        }
+                    const uint32_t bO = __ballot_sync(0xffffffffu, cls == CL_OPEN);
+                    if (lane == 0) {
+                        atomicAdd(&a.counters[OGC_CL_OPEN], (unsigned long long)__popc(bO));
+                        atomicAdd(&a.counters[OGC_CL_ACCEPT], (unsigned long long)__popc(bA));
+                        atomicAdd(&a.counters[OGC_CL_GENERIC], (unsigned long long)__popc(bX));
+                        atomicAdd(&a.counters[OGC_CL_DROP], (unsigned long long)(total - __popc(bA | bX | bO)));
+                        atomicAdd(&a.counters[OGC_BATCHES], 1ull);
                     }
                     for (uint32_t j = 0; j < total; ++j) {
-                        const uint32_t mj = __shfl_sync(0xffffffffu, mk, j);
+                        const uint32_t mj = __shfl_sync(0xffffffffu, imask, j);
                         const int cj = __shfl_sync(0xffffffffu, cls, j);
                         if ((mj & mybit) && (cj == CL_OPEN || cj == CL_ACCEPT)) ++c_full;
                         if ((mj & mybit) && cj == CL_DROP) ++c_cull;
                     }
                 }
-                // class A: every target in the mask accepts; only the cutoff is per lane
-#pragma unroll 2
-                for (uint32_t j = 0; j < nA; ++j) {
-                    if (w.an_mask[j] & mybit) {
-                        const float4 s = w.an_com[j];
-                        const float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
-                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        if (r2 < c.rcut2_hi) {
-                            bool in = r2 < c.rcut2_lo;
-                            if (!in) in = og_inside_rcut64(s.x, s.y, s.z, t, c, cnt);
-                            if (in) {
-                                og_monopole_core<POT>(s.w, dx, dy, dz, r2, c, s_tab, acc);
-                                if (COUNT) ++c_ain;
-                            }
-                        }
-                    }
-                }
-                // class X: per-lane decision.  Fast test on (s', G M, lhs, near2, cull2); anything within the
-                // band of a threshold, or where a guard could fire, takes the exact out-of-line visit.
-                uint32_t myopen = 0;
-                for (uint32_t j = 0; j < nX; ++j) {
-                    bool open = false;
-                    if (w.xn_mask[j] & mybit) {
-                        const float4 s = w.xn_com[j];
-                        const float4 x = w.xn_aux[j];
-                        float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
-                        if (x.w != 0.0f) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
-                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        if (r2 > x.z) {
-                            if (COUNT) ++c_cull;
-                        } else {
-                            if (COUNT) ++c_full;
-                            const float rhs = GEOM ? c.theta2 * r2 : t.A * r2 * r2;
-                            const float diff = x.x - rhs, band = OG_BAND * x.x;
-                            if (diff > band) {
-                                open = true;
-                            } else if (diff < -band && r2 > x.y && r2 > hi2m) {
-                                if (r2 < c.rcut2_hi) {
-                                    bool in = r2 < c.rcut2_lo;
-                                    if (!in) in = og_inside_rcut64(s.x, s.y, s.z, t, c, cnt);
-                                    if (in) {
-                                        og_monopole_core<POT>(s.w, dx, dy, dz, r2, c, s_tab, acc);
-                                        if (COUNT) ++c_ain;
+                // undecided nodes: per-lane test.  Fast path on (s', GM, lhs, near2, cull2, band); a lane that
+                // could be inside a guard region evaluates the guards from the staged cell; anything within
+                // the band of a threshold takes the exact out-of-line decision.
+                uint32_t accw = 0u, myopen = 0u;
+                {
+                    const bool xwrap = (bX & bW) != 0u;
+                    uint32_t rem = bX;
+                    while (rem) {
+                        const int j = __ffs(rem) - 1;
+                        rem &= rem - 1u;
+                        bool open = false;
+                        if ((Mt >> j) & 1u) {
+                            const float4 s = w.xn_com[j];
+                            const float4 x = w.xn_aux[j];
+                            float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
+                            if (xwrap) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
+                            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                            if (r2 > x.z) {
+                                if (COUNT) ++c_cull;
+                            } else {
+                                const float rhs = GEOM ? c.theta2 * r2 : t.A * r2 * r2;
+                                const float diff = x.x - rhs;
+                                bool accept = false;
+                                int counted = 0;
+                                if (diff > x.w) {
+                                    open = true;
+                                } else if (diff < -x.w && r2 > fmaxf(x.y, hi2m)) {
+                                    accept = true;
+                                } else {
+                                    // guards R15 / R16 in fp32 from the staged cell
+                                    const float4 cc = w.xn_cel[j];
+                                    float ex = cc.x - t.x, ey = cc.y - t.y, ez = cc.z - t.z;
+                                    if (xwrap) { ex = og_wrap(ex, c); ey = og_wrap(ey, c); ez = og_wrap(ez, c); }
+                                    const float cmax = fmaxf(fabsf(ex), fmaxf(fabsf(ey), fabsf(ez)));
+                                    const float lim = 0.6f * cc.w;
+                                    const float hh2 = fmaxf(hi2, w.xn_hm2[j]);
+                                    const bool amb = fabsf(diff) <= x.w || fabsf(cmax - lim) <= OG_BAND * cc.w ||
+                                                     fabsf(r2 - hh2) <= OG_BAND * hh2;
+                                    if (amb) {
+                                        const int d = slow_decide<GEOM>(a, w.xn_idx[j], t, cnt);
+                                        open = d == 1; accept = d == 2;
+                                        if (COUNT) { counted = 1; if (d == 0) ++c_cull; else ++c_full; }
+                                    } else {
+                                        open = diff > 0.0f || cmax < lim || r2 < hh2;
+                                        accept = !open;
                                     }
                                 }
-                            } else {
-                                uint32_t n_in = 0;
-                                open = slow_visit<GEOM, POT>(a, w.xn_idx[j], t, s_tab, acc, cnt, n_in);
-                                if (COUNT) c_ain += n_in;
+                                if (COUNT && !counted) ++c_full;
+                                if (accept && r2 < c.rcut2_hi) accw |= 1u << j;
                             }
                         }
+                        const uint32_t b = __ballot_sync(0xffffffffu, open);
+                        if (lane == (uint32_t)j) myopen = b;
                     }
-                    const uint32_t b = __ballot_sync(0xffffffffu, open);
-                    if (cls == CL_GENERIC && pX == j) myopen = b;
+                }
+                if ((bA | bX) != 0u) {
+                    w.W[nseg][lane] = (Mt & bA) | accw;
+                    if (lane == 0) w.seg_flags[nseg] = bW ? SEG_WRAP : 0u;
+                    ++nseg;
                 }
                 __syncwarp();
                 // push opened internal nodes (children ranges) and opened leaves (particle ranges)
                 const uint32_t cmask = (cls == CL_OPEN) ? imask : myopen;
-                const bool is_leaf = (info.y & OG_LEAF_BIT) != 0;
+                const bool is_leaf = (meta >> 26) & 1u;
+                const uint32_t ccount = meta & 0x03ffffffu;
                 const bool push_n = cmask != 0 && !is_leaf;
                 const bool push_p = cmask != 0 && is_leaf;
                 const uint32_t bn = __ballot_sync(0xffffffffu, push_n);
@@ -503,71 +572,73 @@ k_walk_group(WalkArgs a)
                 }
                 if (push_n) {
                     const int p = top + __popc(bn & lt);
-                    w.st_start[p] = info.x; w.st_cnt[p] = info.y; w.st_mask[p] = cmask;
+                    w.st_start[p] = first; w.st_cnt[p] = ccount; w.st_mask[p] = cmask;
                 }
                 top += nn;
                 if (push_p) {
                     const int p = pl_top + __popc(bp & lt);
-                    w.pl_start[p] = info.x; w.pl_cnt[p] = info.y & ~OG_LEAF_BIT; w.pl_mask[p] = cmask;
+                    w.pl_start[p] = first; w.pl_cnt[p] = ccount; w.pl_mask[p] = cmask;
                 }
                 pl_top += __popc(bp);
-                pl_items += __reduce_add_sync(0xffffffffu, push_p ? (info.y & ~OG_LEAF_BIT) : 0u);
+                pl_items += __reduce_add_sync(0xffffffffu, push_p ? ccount : 0u);
                 __syncwarp();
             }
-            // drain the particle list in batches of 32
+            // move the particles of opened leaves into segments, 32 at a time
             while (pl_items >= 32u || (top == 0 && spill_n == 0 && pl_items > 0u)) {
+                if (nseg == GW_NSEG) {
+                    consume<POT, COUNT>(w, nseg, t, c, s_tab, acc, lane, cnt, c_ain, c_pin, c_psoft, c_pout);
+                    nseg = 0;
+                }
                 uint32_t item, imask;
                 const uint32_t total = pop_items(w.pl_start, w.pl_cnt, w.pl_mask, pl_top, lane, item, imask);
                 pl_items -= total;
                 int pc = 0;
-                float4 p;
-                float ph = 0.f;
                 if (lane < total) {
-                    p = __ldg(a.spos + item);
-                    ph = __ldg(a.sh + item);
+                    float4 p = __ldg(a.spos + item);
+                    const float ph = __ldg(a.sh + item);
                     pc = classify_particle(p, g, c);
+                    if (pc != 0) {
+                        p.w *= c.G;
+                        w.ring_pos[nseg * 32 + lane] = p;
+                        w.ring_h[nseg * 32 + lane] = ph;
+                    }
                 }
-                const uint32_t bs = __ballot_sync(0xffffffffu, pc != 0);
-                const uint32_t ns = __popc(bs);
-                if (pc != 0) {
-                    const uint32_t q = __popc(bs & lt);
-                    w.pt_pos[q] = p; w.pt_h[q] = ph; w.pt_slot[q] = item; w.pt_mask[q] = imask; w.pt_flag[q] = (uint32_t)pc;
+                // self exclusion: the lanes whose target IS this particle (target slots ascend with the lane)
+                uint32_t selfm = 0u;
+                {
+                    int lo = 0;
+#pragma unroll
+                    for (int step = 16; step >= 1; step >>= 1) {
+                        const uint32_t v = __shfl_sync(0xffffffffu, t.slot, lo + step - 1);
+                        if (v < item) lo += step;
+                    }
+                    const uint32_t v = __shfl_sync(0xffffffffu, t.slot, lo);
+                    const uint32_t pm = __shfl_sync(0xffffffffu, peers, lo);
+                    if (v == item) selfm = pm;
                 }
-                __syncwarp();
+                const uint32_t b2 = __ballot_sync(0xffffffffu, pc == 2);
+                const uint32_t Mt = transpose32((lane < total && pc != 0) ? (imask & ~selfm) : 0u, lane);
+                w.W[nseg][lane] = Mt;
+                if (lane == 0) w.seg_flags[nseg] = SEG_PART | (b2 ? SEG_WRAP : 0u);
+                ++nseg;
                 if (COUNT) {
-                    const uint32_t b1 = __ballot_sync(0xffffffffu, pc == 1), b2 = __ballot_sync(0xffffffffu, pc == 2);
+                    const uint32_t b1 = __ballot_sync(0xffffffffu, pc == 1);
                     if (lane == 0) {
                         atomicAdd(&a.counters[OGC_PT_SHIFT], (unsigned long long)__popc(b1));
                         atomicAdd(&a.counters[OGC_PT_WRAP], (unsigned long long)__popc(b2));
-                        atomicAdd(&a.counters[OGC_PT_DROP], (unsigned long long)(total - ns));
+                        atomicAdd(&a.counters[OGC_PT_DROP], (unsigned long long)(total - __popc(b1 | b2)));
                     }
                     for (uint32_t j = 0; j < total; ++j) {
-                        const uint32_t mj = __shfl_sync(0xffffffffu, imask, j);
+                        const uint32_t mj = __shfl_sync(0xffffffffu, imask & ~selfm, j);
                         const int cj = __shfl_sync(0xffffffffu, pc, j);
-                        const uint32_t sj = __shfl_sync(0xffffffffu, item, j);
-                        if ((mj & mybit) && cj == 0 && sj != t.slot) ++c_pout;
-                    }
-                }
-#pragma unroll 2
-                for (uint32_t j = 0; j < ns; ++j) {
-                    if ((w.pt_mask[j] & mybit) && w.pt_slot[j] != t.slot) {
-                        const float4 q = w.pt_pos[j];
-                        float dx = q.x - t.x, dy = q.y - t.y, dz = q.z - t.z;
-                        if (w.pt_flag[j] == 2u) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
-                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        int kind = 0;
-                        if (r2 < c.rcut2_hi) {
-                            bool in = r2 < c.rcut2_lo;
-                            if (!in) in = og_inside_rcut64(q.x, q.y, q.z, t, c, cnt);
-                            if (in) kind = og_pair_core<POT>(dx, dy, dz, r2, q.w, w.pt_h[j], t, c, s_tab, acc);
-                        }
-                        if (COUNT) { if (kind == 0) ++c_pout; else { ++c_pin; if (kind == 2) ++c_psoft; } }
+                        if ((mj & mybit) && cj == 0) ++c_pout;
                     }
                 }
                 __syncwarp();
             }
             if (top == 0 && spill_n == 0 && pl_items == 0u) break;
         }
+        if (nseg > 0) consume<POT, COUNT>(w, nseg, t, c, s_tab, acc, lane, cnt, c_ain, c_pin, c_psoft, c_pout);
         if (valid) {
             a.acc_out[3 * (size_t)out] = acc.ax;
             a.acc_out[3 * (size_t)out + 1] = acc.ay;
@@ -644,7 +715,7 @@ cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t 
 {
     WalkArgs a;
     a.com = t->node_com; a.cell = t->node_cell; a.lo = t->node_lo; a.hi = t->node_hi;
-    a.info = t->node_info; a.spos = t->spos; a.sh = t->sh; a.tab = t->split_tab;
+    a.info = t->node_info; a.n1 = t->node_n1; a.n2 = t->node_n2; a.spos = t->spos; a.sh = t->sh; a.tab = t->split_tab;
     a.tgt_slot = tgt_slot; a.tgt_out = tgt_out; a.a_old = a_old; a.acc_out = acc_out; a.pot_out = pot_out;
     a.n_active = (uint32_t)n_active;
     a.n_groups = (uint32_t)((n_active + 31) / 32);

@@ -83,10 +83,11 @@ __device__ __forceinline__ bool og_inside_rcut(float r2, float sx, float sy, flo
 }
 
 // ---- pair kernel C5 ------------------------------------------------------------------------
-// Interaction with a source particle at nearest-image offset d (|d|^2 = r2, already known to be
-// inside r_cut), mass pm, softening length ph.  Returns 1 for r >= h, 2 for r < h.
+// Interaction with a source at nearest-image offset d (|d|^2 = r2, already known to be inside
+// r_cut), gm = G * mass, softening length ph (0 for a node monopole: R16 guarantees r >= h_i there,
+// so node interactions are Newtonian, R21).  Returns 1 for r >= h, 2 for r < h.
 template <bool POT>
-__device__ __forceinline__ int og_pair_core(float dx, float dy, float dz, float r2, float pm, float ph,
+__device__ __forceinline__ int og_pair_core(float dx, float dy, float dz, float r2, float gm, float ph,
                                             const Target &t, const WalkConst &c,
                                             const float4 *__restrict__ tab, Accum &acc)
 {
@@ -119,7 +120,6 @@ __device__ __forceinline__ int og_pair_core(float dx, float dy, float dz, float 
                          0.06666666666666667f * uinv);
         }
     }
-    const float gm = c.G * pm;
     const float f = gm * g * T;
     acc.ax = fmaf(f, dx, acc.ax);
     acc.ay = fmaf(f, dy, acc.ay);
@@ -138,7 +138,7 @@ __device__ __forceinline__ int og_pair(const float4 p, float ph, const Target &t
     const float dx = og_wrap(p.x - t.x, c), dy = og_wrap(p.y - t.y, c), dz = og_wrap(p.z - t.z, c);
     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
     if (!og_inside_rcut(r2, p.x, p.y, p.z, t, c, counters)) return 0;
-    return og_pair_core<POT>(dx, dy, dz, r2, p.w, ph, t, c, tab, acc);
+    return og_pair_core<POT>(dx, dy, dz, r2, c.G * p.w, ph, t, c, tab, acc);
 }
 
 // ---- node: cull, opening decision, monopole ------------------------------------------------
