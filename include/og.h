@@ -88,6 +88,7 @@ typedef struct {
      * all / accepted by all / undecided; particles dropped / staged shifted / staged for per-lane
      * wrap; node batches popped                                                              */
     uint64_t cl_drop, cl_open, cl_accept, cl_generic, pt_drop, pt_shift, pt_wrap, batches;
+    uint64_t diag[32];      /* implementation diagnostics of the walk kernel (OG_COUNT); meaning may change */
 } og_stats;
 
 /* og_tree_get field selectors.  Pointers are DEVICE pointers into the tree, valid until

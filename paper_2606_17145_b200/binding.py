@@ -62,10 +62,12 @@ class og_stats(C.Structure):
                 ("P_soft", C.c_uint64), ("P_out", C.c_uint64), ("fp64_rechecks", C.c_uint64),
                 ("cl_drop", C.c_uint64), ("cl_open", C.c_uint64), ("cl_accept", C.c_uint64),
                 ("cl_generic", C.c_uint64), ("pt_drop", C.c_uint64), ("pt_shift", C.c_uint64),
-                ("pt_wrap", C.c_uint64), ("batches", C.c_uint64)]
+                ("pt_wrap", C.c_uint64), ("batches", C.c_uint64), ("diag", C.c_uint64 * 32)]
 
     def as_dict(self):
-        return {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}
+        d = {k: int(getattr(self, k)) for k, _ in self._fields_ if k not in ("reserved", "diag")}
+        d["diag"] = [int(x) for x in self.diag]
+        return d
 
 
 def make_params(r_s, G=1.0, rcut_over_rs=4.5, alpha=0.005, theta=0.5, leaf_max=8, max_nodes=0, flags=OG_PERIODIC,

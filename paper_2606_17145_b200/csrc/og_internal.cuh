@@ -17,7 +17,8 @@
 // Counter slots (og_tree::d_counters), see og_stats.
 enum { OGC_V_FULL = 0, OGC_V_CULL, OGC_A_IN, OGC_P_IN, OGC_P_SOFT, OGC_P_OUT, OGC_FP64,
        // group-walk diagnostics: nodes per class, particles per class, batches
-       OGC_CL_DROP, OGC_CL_OPEN, OGC_CL_ACCEPT, OGC_CL_GENERIC, OGC_PT_DROP, OGC_PT_SHIFT, OGC_PT_WRAP, OGC_BATCHES, OGC_N };
+       OGC_CL_DROP, OGC_CL_OPEN, OGC_CL_ACCEPT, OGC_CL_GENERIC, OGC_PT_DROP, OGC_PT_SHIFT, OGC_PT_WRAP, OGC_BATCHES,
+       OGC_DIAG0, OGC_N = OGC_DIAG0 + 32 };
 
 // Packed node record read by the walk: 4 x float4 + uint2.
 //   com  = (s_x, s_y, s_z, M)                 R9: fp32 rounding of the fp64 upward pass

@@ -316,6 +316,23 @@ __device__ __forceinline__ void consume(WarpSmem &w, int nseg, const Target &t, 
                                         unsigned long long *cnt, uint32_t &c_ain, uint32_t &c_pin,
                                         uint32_t &c_psoft, uint32_t &c_pout)
 {
+    if (COUNT) {   // lane-slots a team-granular evaluation of the accepted sources would need (teams of 1, 4, 8, 16, 32)
+        for (int s = 0; s < nseg; ++s) {
+            const uint32_t col = transpose32(w.W[s][lane], lane);
+            if (col) {
+                const int o = (w.seg_flags[s] & SEG_PART) ? 8 : 0;
+                int n4 = 0, n8 = 0, n16 = 0;
+                for (int q = 0; q < 8; ++q) n4 += ((col >> (4 * q)) & 0xfu) != 0;
+                for (int q = 0; q < 4; ++q) n8 += ((col >> (8 * q)) & 0xffu) != 0;
+                for (int q = 0; q < 2; ++q) n16 += ((col >> (16 * q)) & 0xffffu) != 0;
+                atomicAdd(&cnt[OGC_DIAG0 + o + 0], (unsigned long long)__popc(col));
+                atomicAdd(&cnt[OGC_DIAG0 + o + 1], (unsigned long long)(4 * n4));
+                atomicAdd(&cnt[OGC_DIAG0 + o + 2], (unsigned long long)(8 * n8));
+                atomicAdd(&cnt[OGC_DIAG0 + o + 3], (unsigned long long)(16 * n16));
+                atomicAdd(&cnt[OGC_DIAG0 + o + 4], 32ull);
+            }
+        }
+    }
     int seg = 0;
     uint32_t cur = w.W[0][lane];
     uint32_t fl = w.seg_flags[0];
@@ -460,6 +477,18 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 // Mt: bit j = my target is in the mask of the node lane j holds
                 const uint32_t Mt = transpose32((cls >= CL_ACCEPT) ? imask : 0u, lane);
                 __syncwarp();
+                if (COUNT && cls >= CL_ACCEPT && imask) {   // same for the parent masks of the staged nodes (16: accept, 24: generic)
+                    const int o = (cls == CL_ACCEPT) ? 16 : 24;
+                    int n4 = 0, n8 = 0, n16 = 0;
+                    for (int q = 0; q < 8; ++q) n4 += ((imask >> (4 * q)) & 0xfu) != 0;
+                    for (int q = 0; q < 4; ++q) n8 += ((imask >> (8 * q)) & 0xffu) != 0;
+                    for (int q = 0; q < 2; ++q) n16 += ((imask >> (16 * q)) & 0xffffu) != 0;
+                    atomicAdd(&a.counters[OGC_DIAG0 + o + 0], (unsigned long long)__popc(imask));
+                    atomicAdd(&a.counters[OGC_DIAG0 + o + 1], (unsigned long long)(4 * n4));
+                    atomicAdd(&a.counters[OGC_DIAG0 + o + 2], (unsigned long long)(8 * n8));
+                    atomicAdd(&a.counters[OGC_DIAG0 + o + 3], (unsigned long long)(16 * n16));
+                    atomicAdd(&a.counters[OGC_DIAG0 + o + 4], 32ull);
+                }
                 if (COUNT) {   // group-level outcomes counted as the per-target visits they stand for
                     const uint32_t bO = __ballot_sync(0xffffffffu, cls == CL_OPEN);
                     if (lane == 0) {
