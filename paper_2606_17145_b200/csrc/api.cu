@@ -27,7 +27,7 @@ inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 struct Layout {
     size_t keysA, keysB, idxA, idxB, sort_scratch, spos, sh, inv_perm;
     size_t level, first, count, first_child, nchild, com, cell, lo, hi, info, n1, n2;
-    size_t oct_scratch, level_start, status, counters, split_tab, spill, total;
+    size_t oct_scratch, level_start, status, counters, small_end, spill, total;
 };
 
 Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count)
@@ -49,7 +49,7 @@ Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count)
     L.level_start = take(24 * 4);
     L.status = take(16 * 4);
     L.counters = take(OGC_N * 8);
-    L.split_tab = take(1025 * 16);
+    L.small_end = o;
     L.spill = take(ogk_walk_spill_bytes(sm_count));
     L.total = o;
     return L;
@@ -77,6 +77,10 @@ bool check_params(const og_params *p, uint64_t n, float box)
     if (!(p->flags & OG_PERIODIC)) { og_set_error("OG_PERIODIC is required in this build"); return false; }
     if (p->leaf_max == 0) { og_set_error("leaf_max must be >= 1"); return false; }
     if (!(p->r_s > 0.0f) || !(p->rcut_over_rs > 0.0f)) { og_set_error("r_s and rcut_over_rs must be > 0"); return false; }
+    if (p->rcut_over_rs > 5.0f) {
+        og_set_error("rcut_over_rs = %g > 5: the split-factor polynomial is fitted on r / (2 r_s) <= 2.5", (double)p->rcut_over_rs);
+        return false;
+    }
     if (!((double)p->rcut_over_rs * (double)p->r_s < 0.5 * (double)box)) {
         og_set_error("r_cut = %g must be < box/2 = %g (nearest-image convention, R13)",
                      (double)p->rcut_over_rs * (double)p->r_s, 0.5 * (double)box);
@@ -211,7 +215,6 @@ extern "C" og_tree *og_tree_build(const float *pos, const float *mass, const flo
     t->node_n1 = (uint4 *)(b + L.n1); t->node_n2 = (float4 *)(b + L.n2);
     t->d_level_start = (uint32_t *)(b + L.level_start); t->d_status = (uint32_t *)(b + L.status);
     t->d_counters = (unsigned long long *)(b + L.counters);
-    t->split_tab = (float4 *)(b + L.split_tab);
     t->walk_spill = b + L.spill; t->walk_spill_bytes = ogk_walk_spill_bytes(sms);
 
 #define OG_BUILD_TRY(expr)                                                    \
@@ -221,15 +224,13 @@ extern "C" og_tree *og_tree_build(const float *pos, const float *mass, const flo
         return nullptr;                                                       \
     })
     // level_start, status, counters are adjacent: clear them in one memset
-    OG_BUILD_TRY(cudaMemsetAsync(b + L.level_start, 0, L.split_tab - L.level_start, st));
+    OG_BUILD_TRY(cudaMemsetAsync(b + L.level_start, 0, L.small_end - L.level_start, st));
     OG_BUILD_TRY(ogk_keys(pos, n, box, keysA, idxA, t->d_status, (params->flags & OG_VALIDATE_POS) != 0, st));
     int in_alt = 0;
     OG_BUILD_TRY(ogk_radix_sort(keysA, idxA, keysB, idxB, n, 0, 64, b + L.sort_scratch, &in_alt, st));
     t->keys = in_alt ? keysB : keysA;
     t->perm = in_alt ? idxB : idxA;
     OG_BUILD_TRY(ogk_gather(pos, mass, soft, t->perm, n, t->spos, t->sh, t->inv_perm, st));
-    OG_BUILD_TRY(ogk_split_table(t->split_tab, (double)params->rcut_over_rs * (double)params->r_s,
-                                 (double)params->r_s, st));
     OG_BUILD_TRY(ogk_octree_upward(t, b + L.oct_scratch, st));
 #undef OG_BUILD_TRY
     return t;

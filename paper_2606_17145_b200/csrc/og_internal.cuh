@@ -67,7 +67,6 @@ struct og_tree {
     //   n2 = (c_x, c_y, c_z, h_max)
     uint4 *node_n1;
     float4 *node_n2;
-    float4 *split_tab;         // OG_NTAB rows (T, dT, E, dE), see walk_math.cuh
     // small device state
     uint32_t *d_level_start;   // [24]: start index per level, [22] = n_nodes, [23] = max level
     uint32_t *d_status;        // [4]: latched status bits, walk work counter, ...
@@ -115,7 +114,6 @@ cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t 
                      uint64_t n_active, const float *a_old, float *acc_out, float *pot_out,
                      cudaStream_t st);
 size_t ogk_walk_spill_bytes(int sm_count);
-cudaError_t ogk_split_table(float4 *tab, double rcut, double r_s, cudaStream_t st);
 // helpers for the active subset
 cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_perm, uint64_t n,
                              uint64_t n_active, uint64_t *keys, uint32_t *vals, uint32_t *d_status,

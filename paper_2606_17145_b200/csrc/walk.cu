@@ -14,8 +14,11 @@
 // nodes cost one monopole per lane with no decision work, undecided ones get the exact
 // per-lane cull / opening test and a ballot yields the mask of the children.  Opened leaves go
 // to a second range list whose particles are staged (after a group-level cutoff test and an
-// exact periodic shift) and evaluated in batches of 32.  The split table (T, T', E, E') lives in
-// shared memory.  Results are written straight to the caller's order (a7 fused).
+// exact periodic shift) in segments of 32.  Staged sources live in a shared-memory ring of GW_NSEG
+// segments; every lane walks the set bits of its OWN words W[seg][lane] and may lag up to a whole
+// ring behind the producer, so a lane idles only when it has nothing left in the ring.  The split
+// factors T, E are evaluated in registers (polynomial x ex2, walk_math.cuh).  Results are written
+// straight to the caller's order (a7 fused).
 //
 // k_walk_simple: one thread per target with a private stack; debugging / comparison only.
 #include "walk_math.cuh"
@@ -29,7 +32,6 @@ struct WalkArgs {
     const float4 *n2;          // (c_x, c_y, c_z, h_max)
     const float4 *spos;
     const float *sh;
-    const float4 *tab;
     const uint32_t *tgt_slot;  // NULL -> identity
     const uint32_t *tgt_out;   // position in the caller's order
     const float *a_old;
@@ -69,19 +71,11 @@ __device__ __forceinline__ Target load_target(const WalkArgs &a, uint32_t k, uin
     return t;
 }
 
-__device__ __forceinline__ void copy_table(float4 *s_tab, const float4 *g_tab)
-{
-    for (int i = threadIdx.x; i < OG_NTAB + 1; i += blockDim.x) s_tab[i] = g_tab[i];
-}
-
 // -------------------------------------------------------------------------------------------
 template <bool GEOM, bool POT, bool COUNT>
 __global__ void __launch_bounds__(128)
 k_walk_simple(const __grid_constant__ WalkArgs a)
 {
-    __shared__ float4 s_tab[OG_NTAB + 1];
-    copy_table(s_tab, a.tab);
-    __syncthreads();
     const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= a.n_active) return;
     uint32_t out;
@@ -99,7 +93,7 @@ k_walk_simple(const __grid_constant__ WalkArgs a)
         ++c_full;
         float dx, dy, dz, r2;
         if (!og_open<GEOM>(n, t, a.c, dx, dy, dz, r2, cnt)) {
-            c_ain += og_monopole<POT>(n, t, a.c, s_tab, dx, dy, dz, r2, acc, cnt);
+            c_ain += og_monopole<POT>(n, t, a.c, dx, dy, dz, r2, acc, cnt);
             continue;
         }
         const uint2 info = __ldg(a.info + j);
@@ -107,7 +101,7 @@ k_walk_simple(const __grid_constant__ WalkArgs a)
             const uint32_t f = info.x, c = info.y & ~OG_LEAF_BIT;
             for (uint32_t s = f; s < f + c; ++s) {
                 if (s == t.slot) continue;
-                const int kind = og_pair<POT>(__ldg(a.spos + s), __ldg(a.sh + s), t, a.c, s_tab, acc, cnt);
+                const int kind = og_pair<POT>(__ldg(a.spos + s), __ldg(a.sh + s), t, a.c, acc, cnt);
                 if (kind == 0) ++c_pout; else { ++c_pin; if (kind == 2) ++c_psoft; }
             }
         } else {
@@ -137,9 +131,8 @@ constexpr int GW_THREADS = GW_WARPS * 32;
 constexpr int GW_STACK = 256;         // node-range stack entries per warp in shared memory
 constexpr int GW_SPILL = 128;         // entries moved to / from global memory at a time
 constexpr int GW_PLIST = 64;          // particle-range list entries per warp
-constexpr int GW_NSEG = 8;            // 32-source segments buffered per warp before they are evaluated
+constexpr int GW_NSEG = 8;            // 32-source segments in the per-warp source ring (power of two)
 
-#define SEG_WRAP 1u      // some source of the segment is not pre-shifted: per-lane nearest-image wrap
 #define SEG_PART 2u      // particle segment (else node segment); only the counters care
 
 // Per-warp working set.  Sources (accepted nodes and particles of opened leaves) are
@@ -308,63 +301,108 @@ __device__ __forceinline__ float warp_max_pos(float v)
     return __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(v)));
 }
 
-// Evaluates the buffered segments: every lane walks the set bits of its own words W[seg][lane] and adds
-// the pair kernel C5 for each (nodes are sources with h = 0: the softening guard R16 guarantees r >= h_i).
-template <bool POT, bool COUNT>
-__device__ __forceinline__ void consume(WarpSmem &w, int nseg, const Target &t, const WalkConst &c,
-                                        const float4 *__restrict__ s_tab, Accum &acc, uint32_t lane,
-                                        unsigned long long *cnt, uint32_t &c_ain, uint32_t &c_pin,
-                                        uint32_t &c_psoft, uint32_t &c_pout)
+// Per-lane interaction counters (OG_COUNT builds only).
+struct LaneCount {
+    uint32_t full, cull, ain, pin, psoft, pout;
+};
+
+// One source q = (x', y', z', G m) against the lane's target, exact in every respect: nearest-image wrap,
+// cutoff decision with fp64 band, softened kernel.  Returns (dax, day, daz, dpot); kind = 0 outside r_cut,
+// 1 inside with r >= h, 2 inside with r < h.  Out of line: the fast path below handles everything that is
+// neither within OG_BAND of r_cut nor possibly softened.
+template <bool POT>
+__device__ __noinline__ float4 pair_exact(const float4 q, const float hj, const Target &t, const WalkConst &c,
+                                          unsigned long long *cnt, int &kind)
 {
-    if (COUNT) {   // lane-slots a team-granular evaluation of the accepted sources would need (teams of 1, 4, 8, 16, 32)
-        for (int s = 0; s < nseg; ++s) {
-            const uint32_t col = transpose32(w.W[s][lane], lane);
-            if (col) {
-                const int o = (w.seg_flags[s] & SEG_PART) ? 8 : 0;
-                int n4 = 0, n8 = 0, n16 = 0;
-                for (int q = 0; q < 8; ++q) n4 += ((col >> (4 * q)) & 0xfu) != 0;
-                for (int q = 0; q < 4; ++q) n8 += ((col >> (8 * q)) & 0xffu) != 0;
-                for (int q = 0; q < 2; ++q) n16 += ((col >> (16 * q)) & 0xffffu) != 0;
-                atomicAdd(&cnt[OGC_DIAG0 + o + 0], (unsigned long long)__popc(col));
-                atomicAdd(&cnt[OGC_DIAG0 + o + 1], (unsigned long long)(4 * n4));
-                atomicAdd(&cnt[OGC_DIAG0 + o + 2], (unsigned long long)(8 * n8));
-                atomicAdd(&cnt[OGC_DIAG0 + o + 3], (unsigned long long)(16 * n16));
-                atomicAdd(&cnt[OGC_DIAG0 + o + 4], 32ull);
-            }
-        }
-    }
-    int seg = 0;
-    uint32_t cur = w.W[0][lane];
-    uint32_t fl = w.seg_flags[0];
+    const float dx = og_wrap(q.x - t.x, c), dy = og_wrap(q.y - t.y, c), dz = og_wrap(q.z - t.z, c);
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    Accum d = {0.f, 0.f, 0.f, 0.f};
+    kind = 0;
+    if (og_inside_rcut(r2, q.x, q.y, q.z, t, c, cnt)) kind = og_pair_core<POT>(dx, dy, dz, r2, q.w, hj, t, c, d);
+    return make_float4(d.ax, d.ay, d.az, d.pot);
+}
+
+// Position of a lane in the source ring: `nxt` = next segment (monotone counter) whose word the lane will
+// load, `cur` = bits of segment nxt - 1 it has not evaluated yet, `base` = ring slot of that segment's
+// first source.
+struct LanePos {
+    uint32_t nxt, cur, base, part;   // part: the segment holds particles (counters only)
+};
+
+// Evaluates ring sources until every lane has finished all segments < target (target <= head, the number
+// of segments produced so far).  Every lane walks the set bits of its own words, two sources per
+// iteration (two independent dependency chains).  Newtonian monopole x split factor in the loop (R21);
+// a source that is within OG_BAND of r_cut or closer than the largest softening length of the whole
+// particle set goes to pair_exact.  Returns the number of segments all lanes have finished.
+template <bool POT, bool COUNT, bool WRAP>
+__device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, const uint32_t target, LanePos &lp,
+                                            const Target &t, const float hmax2g, const WalkConst &c, Accum &acc,
+                                            const uint32_t lane, unsigned long long *cnt, LaneCount &lc)
+{
     for (;;) {
-        while (cur == 0u && seg + 1 < nseg) {
-            ++seg;
-            cur = w.W[seg][lane];
-            fl = w.seg_flags[seg];
+        if (lp.cur == 0u && lp.nxt < head) {
+            const uint32_t sl = lp.nxt & (GW_NSEG - 1);
+            lp.cur = w.W[sl][lane];
+            lp.base = sl * 32u;
+            if (COUNT) lp.part = w.seg_flags[sl] & SEG_PART;
+            ++lp.nxt;
         }
-        if (!__any_sync(0xffffffffu, cur != 0u)) break;
-        if (cur != 0u) {
-            const int j = __ffs(cur) - 1;
-            cur &= cur - 1u;
-            const int e = seg * 32 + j;
-            const float4 q = w.ring_pos[e];
-            const float hj = w.ring_h[e];
-            float dx = q.x - t.x, dy = q.y - t.y, dz = q.z - t.z;
-            if (fl & SEG_WRAP) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            int kind = 0;
-            if (r2 < c.rcut2_hi) {
-                bool in = r2 < c.rcut2_lo;
-                if (!in) in = og_inside_rcut64(q.x, q.y, q.z, t, c, cnt);
-                if (in) kind = og_pair_core<POT>(dx, dy, dz, r2, q.w, hj, t, c, s_tab, acc);
+        uint32_t cur = lp.cur;
+        const bool v0 = cur != 0u;
+        const uint32_t e0 = lp.base + ((__ffs(cur) - 1) & 31);
+        cur &= cur - 1u;
+        const bool v1 = cur != 0u;
+        const uint32_t e1 = lp.base + ((__ffs(cur) - 1) & 31);
+        cur &= cur - 1u;
+        lp.cur = cur;
+        const float4 q0 = w.ring_pos[e0], q1 = w.ring_pos[e1];
+        float dx0 = q0.x - t.x, dy0 = q0.y - t.y, dz0 = q0.z - t.z;
+        float dx1 = q1.x - t.x, dy1 = q1.y - t.y, dz1 = q1.z - t.z;
+        if (WRAP) {
+            dx0 = og_wrap(dx0, c); dy0 = og_wrap(dy0, c); dz0 = og_wrap(dz0, c);
+            dx1 = og_wrap(dx1, c); dy1 = og_wrap(dy1, c); dz1 = og_wrap(dz1, c);
+        }
+        const float r20 = fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0));
+        const float r21 = fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1));
+        // fast: strictly inside the cutoff band and beyond every softening length
+        const bool fast0 = v0 && r20 < c.rcut2_lo && r20 >= hmax2g;
+        const bool fast1 = v1 && r21 < c.rcut2_lo && r21 >= hmax2g;
+        const bool slow0 = v0 && !fast0 && r20 < c.rcut2_hi;
+        const bool slow1 = v1 && !fast1 && r21 < c.rcut2_hi;
+        {
+            const float r2a = fmaxf(r20, 1.0e-20f), r2b = fmaxf(r21, 1.0e-20f);
+            const float ria = rsqrtf(r2a), rib = rsqrtf(r2b);
+            float Ta, Ea, Tb, Eb;
+            og_split(r2a * ria, r2a, c, Ta, Ea);
+            og_split(r2b * rib, r2b, c, Tb, Eb);
+            const float gra = (fast0 ? q0.w : 0.0f) * ria, grb = (fast1 ? q1.w : 0.0f) * rib;
+            const float fa = gra * Ta * (ria * ria), fb = grb * Tb * (rib * rib);
+            acc.ax = fmaf(fa, dx0, acc.ax); acc.ay = fmaf(fa, dy0, acc.ay); acc.az = fmaf(fa, dz0, acc.az);
+            acc.ax = fmaf(fb, dx1, acc.ax); acc.ay = fmaf(fb, dy1, acc.ay); acc.az = fmaf(fb, dz1, acc.az);
+            if (POT) { acc.pot = fmaf(-gra, Ea, acc.pot); acc.pot = fmaf(-grb, Eb, acc.pot); }
+        }
+        int k0 = fast0 ? 1 : 0, k1 = fast1 ? 1 : 0;
+        if (slow0 | slow1) {
+            if (slow0) {
+                const float4 d = pair_exact<POT>(q0, w.ring_h[e0], t, c, cnt, k0);
+                acc.ax += d.x; acc.ay += d.y; acc.az += d.z; acc.pot += d.w;
             }
-            if (COUNT) {
-                if (fl & SEG_PART) { if (kind == 0) ++c_pout; else { ++c_pin; if (kind == 2) ++c_psoft; } }
-                else if (kind != 0) ++c_ain;
+            if (slow1) {
+                const float4 d = pair_exact<POT>(q1, w.ring_h[e1], t, c, cnt, k1);
+                acc.ax += d.x; acc.ay += d.y; acc.az += d.z; acc.pot += d.w;
             }
         }
+        if (COUNT) {
+            if (lp.part) {
+                lc.pin += (k0 != 0) + (k1 != 0); lc.psoft += (k0 == 2) + (k1 == 2);
+                lc.pout += (v0 && k0 == 0) + (v1 && k1 == 0);
+            } else {
+                lc.ain += (k0 != 0) + (k1 != 0);
+            }
+        }
+        const uint32_t done = __reduce_min_sync(0xffffffffu, (cur == 0u) ? lp.nxt : lp.nxt - 1u);
+        if (done >= target) return done;
     }
-    __syncwarp();
 }
 
 template <bool GEOM, bool POT, bool COUNT>
@@ -372,10 +410,7 @@ __global__ void __launch_bounds__(GW_THREADS, 2)
 k_walk_group(const __grid_constant__ WalkArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4 *s_tab = reinterpret_cast<float4 *>(smem_raw);
-    WarpSmem *wsm = reinterpret_cast<WarpSmem *>(smem_raw + (OG_NTAB + 1) * sizeof(float4));
-    copy_table(s_tab, a.tab);
-    __syncthreads();
+    WarpSmem *wsm = reinterpret_cast<WarpSmem *>(smem_raw);
     const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
     WarpSmem &w = wsm[wid];
     const uint32_t lt = lanemask_lt();
@@ -384,6 +419,12 @@ k_walk_group(const __grid_constant__ WalkArgs a)
     unsigned long long *cnt = COUNT ? a.counters : nullptr;
     uint32_t *sp_start = a.spill + (size_t)(blockIdx.x * GW_WARPS + wid) * 3 * a.spill_cap;
     uint32_t *sp_cnt = sp_start + a.spill_cap, *sp_mask = sp_cnt + a.spill_cap;
+    // largest softening length of the whole particle set = h_max of the root (R16 / R19 can only matter below it)
+    const float hroot = __ldg(a.lo).w;
+    const float hmax2g = hroot * hroot * (1.0f + OG_BAND);
+    // stale ring slots are read (and masked out) by lanes that have nothing to do: keep them finite
+    for (int i = lane; i < GW_NSEG * 32; i += 32) { w.ring_pos[i] = make_float4(0.f, 0.f, 0.f, 0.f); w.ring_h[i] = 0.f; }
+    __syncwarp();
 
     for (;;) {
         uint32_t gi = 0;
@@ -416,15 +457,28 @@ k_walk_group(const __grid_constant__ WalkArgs a)
         const float hi2 = t.h * t.h;
         const float hi2m = hi2 * (1.0f + OG_GM);   // own softening guard threshold (R16), padded
         Accum acc = {0.f, 0.f, 0.f, 0.f};
-        uint32_t c_full = 0, c_cull = 0, c_ain = 0, c_pin = 0, c_psoft = 0, c_pout = 0;
-        int top = 0, pl_top = 0, nseg = 0;
+        LaneCount lc = {0, 0, 0, 0, 0, 0};
+        int top = 0, pl_top = 0;
         uint32_t pl_items = 0, spill_n = 0;
+        uint32_t head = 0, tail = 0;          // ring: segments produced / finished by all lanes
+        bool anywrap = false;                 // some staged source of this group is not pre-shifted
+        LanePos lp = {0u, 0u, 0u, 0u};
         {
             const uint32_t vm = __ballot_sync(0xffffffffu, valid);
             if (lane == 0) { w.st_start[0] = 0; w.st_cnt[0] = 1; w.st_mask[0] = vm; }
             top = 1;
             __syncwarp();
         }
+        // frees at least half of the ring
+        auto make_room = [&]() {
+            if (head - tail == (uint32_t)GW_NSEG) {
+                __syncwarp();
+                const uint32_t target = tail + GW_NSEG / 2;
+                tail = anywrap ? consume<POT, COUNT, true>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc)
+                               : consume<POT, COUNT, false>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc);
+                __syncwarp();
+            }
+        };
         for (;;) {
             if (top == 0 && spill_n > 0) {  // reload spilled entries
                 const uint32_t m = min(spill_n, (uint32_t)GW_SPILL);
@@ -438,10 +492,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 __syncwarp();
             }
             if (top > 0) {
-                if (nseg == GW_NSEG) {
-                    consume<POT, COUNT>(w, nseg, t, c, s_tab, acc, lane, cnt, c_ain, c_pin, c_psoft, c_pout);
-                    nseg = 0;
-                }
+                make_room();
+                const uint32_t slot0 = (head & (GW_NSEG - 1)) * 32u;
                 uint32_t item, imask;
                 const uint32_t total = pop_items(w.st_start, w.st_cnt, w.st_mask, top, lane, item, imask);
                 uint32_t first = 0, meta = 0;
@@ -458,8 +510,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     cls = classify_node<GEOM>(n0, __uint_as_float(n1.x), __uint_as_float(n1.y), l, g, c, sc, aux,
                                               shifted, kx, ky, kz);
                     if (cls >= CL_ACCEPT) {
-                        w.ring_pos[nseg * 32 + lane] = sc;
-                        w.ring_h[nseg * 32 + lane] = 0.0f;
+                        w.ring_pos[slot0 + lane] = sc;
+                        w.ring_h[slot0 + lane] = 0.0f;
                     }
                     if (cls == CL_GENERIC) {
                         w.xn_com[lane] = sc; w.xn_aux[lane] = aux;
@@ -474,22 +526,23 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 const uint32_t bA = __ballot_sync(0xffffffffu, cls == CL_ACCEPT);
                 const uint32_t bX = __ballot_sync(0xffffffffu, cls == CL_GENERIC);
                 const uint32_t bW = __ballot_sync(0xffffffffu, cls >= CL_ACCEPT && !shifted);
+                anywrap |= bW != 0u;
                 // Mt: bit j = my target is in the mask of the node lane j holds
                 const uint32_t Mt = transpose32((cls >= CL_ACCEPT) ? imask : 0u, lane);
                 __syncwarp();
-                if (COUNT && cls >= CL_ACCEPT && imask) {   // same for the parent masks of the staged nodes (16: accept, 24: generic)
-                    const int o = (cls == CL_ACCEPT) ? 16 : 24;
-                    int n4 = 0, n8 = 0, n16 = 0;
-                    for (int q = 0; q < 8; ++q) n4 += ((imask >> (4 * q)) & 0xfu) != 0;
-                    for (int q = 0; q < 4; ++q) n8 += ((imask >> (8 * q)) & 0xffu) != 0;
-                    for (int q = 0; q < 2; ++q) n16 += ((imask >> (16 * q)) & 0xffffu) != 0;
-                    atomicAdd(&a.counters[OGC_DIAG0 + o + 0], (unsigned long long)__popc(imask));
-                    atomicAdd(&a.counters[OGC_DIAG0 + o + 1], (unsigned long long)(4 * n4));
-                    atomicAdd(&a.counters[OGC_DIAG0 + o + 2], (unsigned long long)(8 * n8));
-                    atomicAdd(&a.counters[OGC_DIAG0 + o + 3], (unsigned long long)(16 * n16));
-                    atomicAdd(&a.counters[OGC_DIAG0 + o + 4], 32ull);
-                }
                 if (COUNT) {   // group-level outcomes counted as the per-target visits they stand for
+                    if (cls >= CL_ACCEPT && imask) {   // diag: lane-slots a team-granular evaluation would need
+                        const int o = (cls == CL_ACCEPT) ? 16 : 24;
+                        int n4 = 0, n8 = 0, n16 = 0;
+                        for (int q = 0; q < 8; ++q) n4 += ((imask >> (4 * q)) & 0xfu) != 0;
+                        for (int q = 0; q < 4; ++q) n8 += ((imask >> (8 * q)) & 0xffu) != 0;
+                        for (int q = 0; q < 2; ++q) n16 += ((imask >> (16 * q)) & 0xffffu) != 0;
+                        atomicAdd(&a.counters[OGC_DIAG0 + o + 0], (unsigned long long)__popc(imask));
+                        atomicAdd(&a.counters[OGC_DIAG0 + o + 1], (unsigned long long)(4 * n4));
+                        atomicAdd(&a.counters[OGC_DIAG0 + o + 2], (unsigned long long)(8 * n8));
+                        atomicAdd(&a.counters[OGC_DIAG0 + o + 3], (unsigned long long)(16 * n16));
+                        atomicAdd(&a.counters[OGC_DIAG0 + o + 4], 32ull);
+                    }
                     const uint32_t bO = __ballot_sync(0xffffffffu, cls == CL_OPEN);
                     if (lane == 0) {
                         atomicAdd(&a.counters[OGC_CL_OPEN], (unsigned long long)__popc(bO));
@@ -501,73 +554,84 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     for (uint32_t j = 0; j < total; ++j) {
                         const uint32_t mj = __shfl_sync(0xffffffffu, imask, j);
                         const int cj = __shfl_sync(0xffffffffu, cls, j);
-                        if ((mj & mybit) && (cj == CL_OPEN || cj == CL_ACCEPT)) ++c_full;
-                        if ((mj & mybit) && cj == CL_DROP) ++c_cull;
+                        if ((mj & mybit) && (cj == CL_OPEN || cj == CL_ACCEPT)) ++lc.full;
+                        if ((mj & mybit) && cj == CL_DROP) ++lc.cull;
                     }
                 }
-                // undecided nodes: per-lane test.  Fast path on (s', GM, lhs, near2, cull2, band); a lane that
-                // could be inside a guard region evaluates the guards from the staged cell; anything within
-                // the band of a threshold takes the exact out-of-line decision.
+                // Undecided nodes: every lane tests every staged node (broadcast LDS) branch-free on
+                // (s', GM, lhs, near2, cull2, band): culled / opens / accepts / needs the guards.  The
+                // few lanes of the last kind then evaluate the guards R15 / R16 from the staged cell, and
+                // anything within the band of a threshold takes the exact out-of-line decision.
                 uint32_t accw = 0u, myopen = 0u;
-                {
+                if (bX != 0u) {
                     const bool xwrap = (bX & bW) != 0u;
+                    uint32_t openw = 0u, sloww = 0u;
                     uint32_t rem = bX;
                     while (rem) {
                         const int j = __ffs(rem) - 1;
                         rem &= rem - 1u;
-                        bool open = false;
-                        if ((Mt >> j) & 1u) {
-                            const float4 s = w.xn_com[j];
-                            const float4 x = w.xn_aux[j];
-                            float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
-                            if (xwrap) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
-                            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                            if (r2 > x.z) {
-                                if (COUNT) ++c_cull;
-                            } else {
-                                const float rhs = GEOM ? c.theta2 * r2 : t.A * r2 * r2;
-                                const float diff = x.x - rhs;
-                                bool accept = false;
-                                int counted = 0;
-                                if (diff > x.w) {
-                                    open = true;
-                                } else if (diff < -x.w && r2 > fmaxf(x.y, hi2m)) {
-                                    accept = true;
-                                } else {
-                                    // guards R15 / R16 in fp32 from the staged cell
-                                    const float4 cc = w.xn_cel[j];
-                                    float ex = cc.x - t.x, ey = cc.y - t.y, ez = cc.z - t.z;
-                                    if (xwrap) { ex = og_wrap(ex, c); ey = og_wrap(ey, c); ez = og_wrap(ez, c); }
-                                    const float cmax = fmaxf(fabsf(ex), fmaxf(fabsf(ey), fabsf(ez)));
-                                    const float lim = 0.6f * cc.w;
-                                    const float hh2 = fmaxf(hi2, w.xn_hm2[j]);
-                                    const bool amb = fabsf(diff) <= x.w || fabsf(cmax - lim) <= OG_BAND * cc.w ||
-                                                     fabsf(r2 - hh2) <= OG_BAND * hh2;
-                                    if (amb) {
-                                        const int d = slow_decide<GEOM>(a, w.xn_idx[j], t, cnt);
-                                        open = d == 1; accept = d == 2;
-                                        if (COUNT) { counted = 1; if (d == 0) ++c_cull; else ++c_full; }
-                                    } else {
-                                        open = diff > 0.0f || cmax < lim || r2 < hh2;
-                                        accept = !open;
-                                    }
-                                }
-                                if (COUNT && !counted) ++c_full;
-                                if (accept && r2 < c.rcut2_hi) accw |= 1u << j;
-                            }
-                        }
-                        const uint32_t b = __ballot_sync(0xffffffffu, open);
-                        if (lane == (uint32_t)j) myopen = b;
+                        const float4 s = w.xn_com[j];
+                        const float4 x = w.xn_aux[j];
+                        float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
+                        if (xwrap) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
+                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                        const float rhs = GEOM ? c.theta2 * r2 : t.A * r2 * r2;
+                        const float diff = x.x - rhs;
+                        const bool inm = (Mt >> j) & 1u;
+                        const bool cand = inm && !(r2 > x.z);
+                        const bool fopen = diff > x.w;
+                        const bool facc = diff < -x.w && r2 > fmaxf(x.y, hi2m);
+                        const uint32_t bit = 1u << j;
+                        if (cand && fopen) openw |= bit;
+                        if (cand && !fopen && facc && r2 < c.rcut2_hi) accw |= bit;
+                        if (cand && !fopen && !facc) sloww |= bit;
+                        if (COUNT) { if (inm && !cand) ++lc.cull; if (cand && (fopen || facc)) ++lc.full; }
                     }
+                    while (sloww) {   // per lane, rare
+                        const int j = __ffs(sloww) - 1;
+                        sloww &= sloww - 1u;
+                        const float4 s = w.xn_com[j];
+                        const float4 x = w.xn_aux[j];
+                        const float4 cc = w.xn_cel[j];
+                        float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
+                        float ex = cc.x - t.x, ey = cc.y - t.y, ez = cc.z - t.z;
+                        if (xwrap) {
+                            dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c);
+                            ex = og_wrap(ex, c); ey = og_wrap(ey, c); ez = og_wrap(ez, c);
+                        }
+                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                        const float rhs = GEOM ? c.theta2 * r2 : t.A * r2 * r2;
+                        const float diff = x.x - rhs;
+                        const float cmax = fmaxf(fabsf(ex), fmaxf(fabsf(ey), fabsf(ez)));
+                        const float lim = 0.6f * cc.w;
+                        const float hh2 = fmaxf(hi2, w.xn_hm2[j]);
+                        const bool amb = fabsf(diff) <= x.w || fabsf(cmax - lim) <= OG_BAND * cc.w ||
+                                         fabsf(r2 - hh2) <= OG_BAND * hh2;
+                        bool open, accept;
+                        if (amb) {
+                            const int d = slow_decide<GEOM>(a, w.xn_idx[j], t, cnt);
+                            open = d == 1; accept = d == 2;
+                            if (COUNT) { if (d == 0) ++lc.cull; else ++lc.full; }
+                        } else {
+                            open = diff > 0.0f || cmax < lim || r2 < hh2;
+                            accept = !open;
+                            if (COUNT) ++lc.full;
+                        }
+                        const uint32_t bit = 1u << j;
+                        if (open) openw |= bit;
+                        if (accept && r2 < c.rcut2_hi) accw |= bit;
+                    }
+                    __syncwarp();
+                    myopen = transpose32(openw, lane);   // lane j: the lanes that open the node lane j holds
                 }
                 if ((bA | bX) != 0u) {
-                    w.W[nseg][lane] = (Mt & bA) | accw;
-                    if (lane == 0) w.seg_flags[nseg] = bW ? SEG_WRAP : 0u;
-                    ++nseg;
+                    w.W[head & (GW_NSEG - 1)][lane] = (Mt & bA) | accw;
+                    if (COUNT && lane == 0) w.seg_flags[head & (GW_NSEG - 1)] = 0u;
+                    ++head;
                 }
                 __syncwarp();
                 // push opened internal nodes (children ranges) and opened leaves (particle ranges)
-                const uint32_t cmask = (cls == CL_OPEN) ? imask : myopen;
+                const uint32_t cmask = (cls == CL_OPEN) ? imask : ((cls == CL_GENERIC) ? myopen : 0u);
                 const bool is_leaf = (meta >> 26) & 1u;
                 const uint32_t ccount = meta & 0x03ffffffu;
                 const bool push_n = cmask != 0 && !is_leaf;
@@ -614,10 +678,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
             }
             // move the particles of opened leaves into segments, 32 at a time
             while (pl_items >= 32u || (top == 0 && spill_n == 0 && pl_items > 0u)) {
-                if (nseg == GW_NSEG) {
-                    consume<POT, COUNT>(w, nseg, t, c, s_tab, acc, lane, cnt, c_ain, c_pin, c_psoft, c_pout);
-                    nseg = 0;
-                }
+                make_room();
+                const uint32_t slot0 = (head & (GW_NSEG - 1)) * 32u;
                 uint32_t item, imask;
                 const uint32_t total = pop_items(w.pl_start, w.pl_cnt, w.pl_mask, pl_top, lane, item, imask);
                 pl_items -= total;
@@ -628,8 +690,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     pc = classify_particle(p, g, c);
                     if (pc != 0) {
                         p.w *= c.G;
-                        w.ring_pos[nseg * 32 + lane] = p;
-                        w.ring_h[nseg * 32 + lane] = ph;
+                        w.ring_pos[slot0 + lane] = p;
+                        w.ring_h[slot0 + lane] = ph;
                     }
                 }
                 // self exclusion: the lanes whose target IS this particle (target slots ascend with the lane)
@@ -646,10 +708,11 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     if (v == item) selfm = pm;
                 }
                 const uint32_t b2 = __ballot_sync(0xffffffffu, pc == 2);
+                anywrap |= b2 != 0u;
                 const uint32_t Mt = transpose32((lane < total && pc != 0) ? (imask & ~selfm) : 0u, lane);
-                w.W[nseg][lane] = Mt;
-                if (lane == 0) w.seg_flags[nseg] = SEG_PART | (b2 ? SEG_WRAP : 0u);
-                ++nseg;
+                w.W[head & (GW_NSEG - 1)][lane] = Mt;
+                if (COUNT && lane == 0) w.seg_flags[head & (GW_NSEG - 1)] = SEG_PART;
+                ++head;
                 if (COUNT) {
                     const uint32_t b1 = __ballot_sync(0xffffffffu, pc == 1);
                     if (lane == 0) {
@@ -660,14 +723,19 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     for (uint32_t j = 0; j < total; ++j) {
                         const uint32_t mj = __shfl_sync(0xffffffffu, imask & ~selfm, j);
                         const int cj = __shfl_sync(0xffffffffu, pc, j);
-                        if ((mj & mybit) && cj == 0) ++c_pout;
+                        if ((mj & mybit) && cj == 0) ++lc.pout;
                     }
                 }
                 __syncwarp();
             }
             if (top == 0 && spill_n == 0 && pl_items == 0u) break;
         }
-        if (nseg > 0) consume<POT, COUNT>(w, nseg, t, c, s_tab, acc, lane, cnt, c_ain, c_pin, c_psoft, c_pout);
+        if (head != tail) {   // drain
+            __syncwarp();
+            if (anywrap) consume<POT, COUNT, true>(w, head, head, lp, t, hmax2g, c, acc, lane, cnt, lc);
+            else consume<POT, COUNT, false>(w, head, head, lp, t, hmax2g, c, acc, lane, cnt, lc);
+            __syncwarp();
+        }
         if (valid) {
             a.acc_out[3 * (size_t)out] = acc.ax;
             a.acc_out[3 * (size_t)out + 1] = acc.ay;
@@ -675,7 +743,7 @@ k_walk_group(const __grid_constant__ WalkArgs a)
             if (POT) a.pot_out[out] = acc.pot;
         }
         if (COUNT) {
-            const uint32_t v[6] = {c_full, c_cull, c_ain, c_pin, c_psoft, c_pout};
+            const uint32_t v[6] = {lc.full, lc.cull, lc.ain, lc.pin, lc.psoft, lc.pout};
             const int slot[6] = {OGC_V_FULL, OGC_V_CULL, OGC_A_IN, OGC_P_IN, OGC_P_SOFT, OGC_P_OUT};
 #pragma unroll
             for (int q = 0; q < 6; ++q) {
@@ -686,22 +754,6 @@ k_walk_group(const __grid_constant__ WalkArgs a)
     }
 }
 
-// split table rows (T, T' dw, E, E' dw) at the nodes w_i = i dw, dw = r_cut / OG_NTAB / (2 r_s), in
-// fp64, stored fp32 (R18).  T' = -(4 w^2 / sqrt(pi)) exp(-w^2), E' = -(2 / sqrt(pi)) exp(-w^2).
-__global__ void k_split_table(float4 *tab, double rcut, double r_s)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i > OG_NTAB) return;
-    const double two_over_sqrt_pi = 1.1283791670955125738961589031215;
-    const double dw = rcut / OG_NTAB / (2.0 * r_s);
-    const double w = (double)i * dw;
-    const double ex = exp(-w * w);
-    const double T = erfc(w) + two_over_sqrt_pi * w * ex;
-    const double dT = -2.0 * two_over_sqrt_pi * w * w * ex * dw;
-    const double E = erfc(w), dE = -two_over_sqrt_pi * ex * dw;
-    tab[i] = make_float4((float)T, (float)dT, (float)E, (float)dE);
-}
-
 template <bool GEOM, bool POT, bool COUNT>
 cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
 {
@@ -710,7 +762,7 @@ cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
         k_walk_simple<GEOM, POT, COUNT><<<grid, 128, 0, st>>>(a);
         return cudaGetLastError();
     }
-    const size_t smem = (OG_NTAB + 1) * sizeof(float4) + GW_WARPS * sizeof(WarpSmem);
+    const size_t smem = GW_WARPS * sizeof(WarpSmem);
     auto kern = k_walk_group<GEOM, POT, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -733,18 +785,12 @@ size_t ogk_walk_spill_bytes(int sm_count)
     return (size_t)sm_count * 4 * GW_WARPS * 3 * SPILL_CAP * sizeof(uint32_t);
 }
 
-cudaError_t ogk_split_table(float4 *tab, double rcut, double r_s, cudaStream_t st)
-{
-    k_split_table<<<(OG_NTAB + 256) / 256, 256, 0, st>>>(tab, rcut, r_s);
-    return cudaGetLastError();
-}
-
 cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out, uint64_t n_active,
                      const float *a_old, float *acc_out, float *pot_out, cudaStream_t st)
 {
     WalkArgs a;
     a.com = t->node_com; a.cell = t->node_cell; a.lo = t->node_lo; a.hi = t->node_hi;
-    a.info = t->node_info; a.n1 = t->node_n1; a.n2 = t->node_n2; a.spos = t->spos; a.sh = t->sh; a.tab = t->split_tab;
+    a.info = t->node_info; a.n1 = t->node_n1; a.n2 = t->node_n2; a.spos = t->spos; a.sh = t->sh;
     a.tgt_slot = tgt_slot; a.tgt_out = tgt_out; a.a_old = a_old; a.acc_out = acc_out; a.pot_out = pot_out;
     a.n_active = (uint32_t)n_active;
     a.n_groups = (uint32_t)((n_active + 31) / 32);
@@ -763,7 +809,9 @@ cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t 
     c.rcut2_lo = c.rcut2 * (1.0f - OG_BAND); c.rcut2_hi = c.rcut2 * (1.0f + OG_BAND);
     c.cull_r = (float)(c.drcut * (1.0 + 1e-5) + 1e-6 * c.dL);
     c.G = p.G; c.alpha = p.alpha; c.theta2 = (float)c.dtheta2;
-    c.tab_scale = (float)((double)OG_NTAB / c.drcut);
+    c.k_w = (float)(0.5 / (double)p.r_s);
+    c.k_e = (float)(-1.4426950408889634 / (4.0 * (double)p.r_s * (double)p.r_s));
+    c.hmax2g = 0.0f;   // read from the root record by the kernels
     cudaError_t e = cudaMemsetAsync(t->d_status + 1, 0, sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
     const bool count = (p.flags & OG_COUNT) != 0;

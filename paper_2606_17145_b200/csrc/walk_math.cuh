@@ -11,7 +11,7 @@
 #include "og_internal.cuh"
 
 #define OG_BAND 1.0e-5f
-#define OG_NTAB 1024  // intervals of the split table on [0, r_cut]; OG_NTAB + 1 rows
+#define OG_WMAX 2.5f  // the split-factor polynomial is fitted on w = r / (2 r_s) in [0, OG_WMAX]: rcut_over_rs <= 5
 
 struct WalkConst {
     float L, invL;
@@ -21,7 +21,9 @@ struct WalkConst {
     float G;
     float alpha;
     float theta2;
-    float tab_scale;     // OG_NTAB / r_cut
+    float k_w;           // 1 / (2 r_s): w = r k_w
+    float k_e;           // -log2(e) / (4 r_s^2): exp(-w^2) = ex2(r^2 k_e)
+    float hmax2g;        // (largest softening length h of any particle)^2 (1 + 1e-5): r^2 above it is Newtonian
     // fp64 copies for the re-evaluation path (C0: fp32 parameters promoted to fp64)
     double dL, drcut, dG, dalpha, dtheta2;
 };
@@ -45,21 +47,33 @@ __device__ __forceinline__ float og_wrap(float d, const WalkConst &c)
 
 __device__ __forceinline__ double og_wrap64(double d, double L) { return d - L * round(d / L); }
 
-// (T, T', E, E') rows in shared memory: T(w) = erfc(w) + 2w/sqrt(pi) exp(-w^2), E = erfc(w),
-// w = r / (2 r_s), tabulated at the OG_NTAB + 1 nodes t = r * OG_NTAB / r_cut = 0..OG_NTAB with the
-// derivative per table step; evaluated as value + (t - nearest node) * derivative (R18; error
-// <= step^2/8 max|T''| ~ 8e-7).  The nearest node comes from the float rounding of t + 1.5 * 2^23
-// (no F2I / I2F in the hot loop).
-__device__ __forceinline__ void og_split(const float4 *__restrict__ tab, float r, const WalkConst &c,
-                                         float &T, float &E)
+// Split factors (R18) in registers: E(w) = erfc(w) = exp(-w^2) P(w), T(w) = E(w) + (2 / sqrt(pi)) w exp(-w^2),
+// w = r / (2 r_s).  P = degree-10 polynomial, weighted-minimax fit of erfcx on [0, OG_WMAX] (weight exp(-w^2));
+// exp(-w^2) = ex2.approx(r^2 k_e).  Max abs error of T and E in fp32 Horner: 1.8e-7 (budget 1e-6).
+__device__ __forceinline__ float og_ex2(float x)
 {
-    const float MAGIC = 12582912.0f;
-    const float tf = fmaf(r, c.tab_scale, MAGIC);
-    const int i = min(__float_as_int(tf) & 0x7ff, OG_NTAB);
-    const float f = fmaf(r, c.tab_scale, MAGIC - tf);
-    const float4 row = tab[i];
-    T = fmaf(f, row.y, row.x);
-    E = fmaf(f, row.w, row.z);
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ void og_split(float r, float r2, const WalkConst &c, float &T, float &E)
+{
+    const float w = r * c.k_w;
+    const float ex = og_ex2(r2 * c.k_e);
+    float p = 1.651949088e-04f;
+    p = fmaf(p, w, -2.225770333e-03f);
+    p = fmaf(p, w, 1.362162625e-02f);
+    p = fmaf(p, w, -5.118135848e-02f);
+    p = fmaf(p, w, 1.361394758e-01f);
+    p = fmaf(p, w, -2.828231287e-01f);
+    p = fmaf(p, w, 4.931623193e-01f);
+    p = fmaf(p, w, -7.507289497e-01f);
+    p = fmaf(p, w, 9.998254850e-01f);
+    p = fmaf(p, w, -1.128371385e+00f);
+    p = fmaf(p, w, 9.999999427e-01f);
+    E = p * ex;
+    T = fmaf(1.1283791670955126f * w, ex, E);
 }
 
 // ---- cutoff decision r < r_cut (R17, strict) ------------------------------------------------
@@ -88,15 +102,14 @@ __device__ __forceinline__ bool og_inside_rcut(float r2, float sx, float sy, flo
 // so node interactions are Newtonian, R21).  Returns 1 for r >= h, 2 for r < h.
 template <bool POT>
 __device__ __forceinline__ int og_pair_core(float dx, float dy, float dz, float r2, float gm, float ph,
-                                            const Target &t, const WalkConst &c,
-                                            const float4 *__restrict__ tab, Accum &acc)
+                                            const Target &t, const WalkConst &c, Accum &acc)
 {
     r2 = fmaxf(r2, 1.0e-36f);           // distinct coincident particles: force 0, potential -14/5 m/h
     const float rinv = rsqrtf(r2);
     const float r = r2 * rinv;
     const float h = fmaxf(t.h, ph);     // R19
     float T, E;
-    og_split(tab, r, c, T, E);
+    og_split(r, r2, c, T, E);
     float g, pp;
     int kind = 1;
     if (r >= h) {
@@ -132,13 +145,12 @@ __device__ __forceinline__ int og_pair_core(float dx, float dy, float dz, float 
 // outside, 1 inside with r >= h, 2 inside with r < h.
 template <bool POT>
 __device__ __forceinline__ int og_pair(const float4 p, float ph, const Target &t, const WalkConst &c,
-                                       const float4 *__restrict__ tab, Accum &acc,
-                                       unsigned long long *counters)
+                                       Accum &acc, unsigned long long *counters)
 {
     const float dx = og_wrap(p.x - t.x, c), dy = og_wrap(p.y - t.y, c), dz = og_wrap(p.z - t.z, c);
     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
     if (!og_inside_rcut(r2, p.x, p.y, p.z, t, c, counters)) return 0;
-    return og_pair_core<POT>(dx, dy, dz, r2, c.G * p.w, ph, t, c, tab, acc);
+    return og_pair_core<POT>(dx, dy, dz, r2, c.G * p.w, ph, t, c, acc);
 }
 
 // ---- node: cull, opening decision, monopole ------------------------------------------------
@@ -234,12 +246,12 @@ __device__ __forceinline__ bool og_open(const NodeRec &n, const Target &t, const
 // factor (R21).
 template <bool POT>
 __device__ __forceinline__ void og_monopole_core(float GM, float dx, float dy, float dz, float r2,
-                                                 const WalkConst &c, const float4 *__restrict__ tab, Accum &acc)
+                                                 const WalkConst &c, Accum &acc)
 {
     const float rinv = rsqrtf(r2);
     const float r = r2 * rinv;
     float T, E;
-    og_split(tab, r, c, T, E);
+    og_split(r, r2, c, T, E);
     const float gr = GM * rinv;
     const float f = gr * T * (rinv * rinv);
     acc.ax = fmaf(f, dx, acc.ax);
@@ -252,10 +264,10 @@ __device__ __forceinline__ void og_monopole_core(float GM, float dx, float dy, f
 // r < r_cut.
 template <bool POT>
 __device__ __forceinline__ int og_monopole(const NodeRec &n, const Target &t, const WalkConst &c,
-                                           const float4 *__restrict__ tab, float dx, float dy, float dz,
+                                           float dx, float dy, float dz,
                                            float r2, Accum &acc, unsigned long long *counters)
 {
     if (!og_inside_rcut(r2, n.com.x, n.com.y, n.com.z, t, c, counters)) return 0;
-    og_monopole_core<POT>(c.G * n.com.w, dx, dy, dz, r2, c, tab, acc);
+    og_monopole_core<POT>(c.G * n.com.w, dx, dy, dz, r2, c, acc);
     return 1;
 }
