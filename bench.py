@@ -39,7 +39,7 @@ from paper_2606_17145_b200 import workloads as W  # noqa: E402
 METRIC = "short-range tree-gravity particles/s (tree build + walk, 1 step) on B200"
 UNIT = "particles/s"
 SM_LANES = 128          # FP32 lanes per SM (B200)
-KERNELS_PER_BUILD = 1 + 8 * 3 + 1 + 1 + 2   # keys, 8 x (hist, scan, scatter), gather, split table, octree + upward
+KERNELS_PER_BUILD = 1 + 8 * 3 + 1 + 2   # keys, 8 x (hist, scan, scatter), gather, octree + upward
 KERNELS_PER_WALK_ALL = 1
 
 
@@ -49,6 +49,20 @@ def load_units(name):
         return None
     with open(p) as f:
         return json.load(f).get(name)
+
+
+def ncu_traffic(name):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one k_walk_group launch on workload `name`, taken from the
+    committed ncu --set full summary profiles/walk_traffic_<name>.txt (line "dram_bytes_per_launch <bytes>")."""
+    p = os.path.join(ROOT, "profiles", f"walk_traffic_{name}.txt")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            tok = line.split()
+            if len(tok) >= 2 and tok[0] == "dram_bytes_per_launch":
+                return float(tok[1])
+    return None
 
 
 def measured_peaks():
@@ -349,7 +363,7 @@ def run_ours(args):
     t_hbm_ms = (units["compulsory_hbm_bytes"] if units else 0) / (float(peaks["hbm_gbs"]) * 1e9) * 1e3
     roofline = {
         "bound": "alu", "kernel": "k_walk_group", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved / peak_tflops, "traffic": None,
+        "frac": achieved / peak_tflops, "traffic": ncu_traffic(w.name),
         "peak_source": f"{sms} SMs x {SM_LANES} FP32 lanes x 2 flop x {fmax / 1e6:.0f} MHz (max SM clock, "
                        f"MEASURED_PEAKS.json {peaks_src}); DESIGN.md Sec. 7",
         "algorithmic_flops_per_launch": F_alg, "units": units_src,

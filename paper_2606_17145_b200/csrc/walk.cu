@@ -126,12 +126,24 @@ k_walk_simple(const __grid_constant__ WalkArgs a)
 }
 
 // -------------------------------------------------------------------------------------------
-constexpr int GW_WARPS = 8;           // warps per block
+#ifndef OG_GW_WARPS
+#define OG_GW_WARPS 8
+#endif
+#ifndef OG_GW_MINBLOCKS
+#define OG_GW_MINBLOCKS 2
+#endif
+#ifndef OG_GW_NSEG
+#define OG_GW_NSEG 8
+#endif
+#ifndef OG_GW_STACK
+#define OG_GW_STACK 256
+#endif
+constexpr int GW_WARPS = OG_GW_WARPS;           // warps per block
 constexpr int GW_THREADS = GW_WARPS * 32;
-constexpr int GW_STACK = 256;         // node-range stack entries per warp in shared memory
-constexpr int GW_SPILL = 128;         // entries moved to / from global memory at a time
+constexpr int GW_STACK = OG_GW_STACK;         // node-range stack entries per warp in shared memory
+constexpr int GW_SPILL = GW_STACK / 2;        // entries moved to / from global memory at a time
 constexpr int GW_PLIST = 64;          // particle-range list entries per warp
-constexpr int GW_NSEG = 8;            // 32-source segments in the per-warp source ring (power of two)
+constexpr int GW_NSEG = OG_GW_NSEG;            // 32-source segments in the per-warp source ring (power of two)
 
 #define SEG_PART 2u      // particle segment (else node segment); only the counters care
 
@@ -371,7 +383,7 @@ __device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, co
         const bool slow1 = v1 && !fast1 && r21 < c.rcut2_hi;
         {
             const float r2a = fmaxf(r20, 1.0e-20f), r2b = fmaxf(r21, 1.0e-20f);
-            const float ria = rsqrtf(r2a), rib = rsqrtf(r2b);
+            const float ria = og_rsqrt(r2a), rib = og_rsqrt(r2b);
             float Ta, Ea, Tb, Eb;
             og_split(r2a * ria, r2a, c, Ta, Ea);
             og_split(r2b * rib, r2b, c, Tb, Eb);
@@ -406,7 +418,7 @@ __device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, co
 }
 
 template <bool GEOM, bool POT, bool COUNT>
-__global__ void __launch_bounds__(GW_THREADS, 2)
+__global__ void __launch_bounds__(GW_THREADS, OG_GW_MINBLOCKS)
 k_walk_group(const __grid_constant__ WalkArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -469,16 +481,6 @@ k_walk_group(const __grid_constant__ WalkArgs a)
             top = 1;
             __syncwarp();
         }
-        // frees at least half of the ring
-        auto make_room = [&]() {
-            if (head - tail == (uint32_t)GW_NSEG) {
-                __syncwarp();
-                const uint32_t target = tail + GW_NSEG / 2;
-                tail = anywrap ? consume<POT, COUNT, true>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc)
-                               : consume<POT, COUNT, false>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc);
-                __syncwarp();
-            }
-        };
         for (;;) {
             if (top == 0 && spill_n > 0) {  // reload spilled entries
                 const uint32_t m = min(spill_n, (uint32_t)GW_SPILL);
@@ -491,8 +493,19 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 top = (int)m;
                 __syncwarp();
             }
-            if (top > 0) {
-                make_room();
+            // next action: a segment of particles of opened leaves, else a batch of nodes, else finish
+            const bool parts = pl_items >= 32u || (top == 0 && pl_items > 0u);
+            const bool fin = top == 0 && pl_items == 0u;
+            if (head - tail == (uint32_t)GW_NSEG || (fin && head != tail)) {
+                // ring full: free at least half of it; finishing: drain it
+                __syncwarp();
+                const uint32_t target = fin ? head : tail + GW_NSEG / 2;
+                tail = anywrap ? consume<POT, COUNT, true>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc)
+                               : consume<POT, COUNT, false>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc);
+                __syncwarp();
+            }
+            if (fin) break;
+            if (!parts) {
                 const uint32_t slot0 = (head & (GW_NSEG - 1)) * 32u;
                 uint32_t item, imask;
                 const uint32_t total = pop_items(w.st_start, w.st_cnt, w.st_mask, top, lane, item, imask);
@@ -675,10 +688,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 pl_top += __popc(bp);
                 pl_items += __reduce_add_sync(0xffffffffu, push_p ? ccount : 0u);
                 __syncwarp();
-            }
-            // move the particles of opened leaves into segments, 32 at a time
-            while (pl_items >= 32u || (top == 0 && spill_n == 0 && pl_items > 0u)) {
-                make_room();
+            } else {
+                // move 32 particles of opened leaves into a segment
                 const uint32_t slot0 = (head & (GW_NSEG - 1)) * 32u;
                 uint32_t item, imask;
                 const uint32_t total = pop_items(w.pl_start, w.pl_cnt, w.pl_mask, pl_top, lane, item, imask);
@@ -728,13 +739,6 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 }
                 __syncwarp();
             }
-            if (top == 0 && spill_n == 0 && pl_items == 0u) break;
-        }
-        if (head != tail) {   // drain
-            __syncwarp();
-            if (anywrap) consume<POT, COUNT, true>(w, head, head, lp, t, hmax2g, c, acc, lane, cnt, lc);
-            else consume<POT, COUNT, false>(w, head, head, lp, t, hmax2g, c, acc, lane, cnt, lc);
-            __syncwarp();
         }
         if (valid) {
             a.acc_out[3 * (size_t)out] = acc.ax;
@@ -770,7 +774,7 @@ cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, GW_THREADS, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
-    if (per_sm > 4) per_sm = 4;   // spill slabs are sized for <= 4 blocks per SM
+    if (per_sm * GW_WARPS > 32) per_sm = 32 / GW_WARPS;   // spill slabs are sized for <= 32 warps per SM
     const unsigned grid = (unsigned)(per_sm * t->sm_count);
     kern<<<grid, GW_THREADS, smem, st>>>(a);
     return cudaGetLastError();
@@ -782,7 +786,7 @@ static constexpr uint32_t SPILL_CAP = 3072;  // entries per warp (x 12 B)
 
 size_t ogk_walk_spill_bytes(int sm_count)
 {
-    return (size_t)sm_count * 4 * GW_WARPS * 3 * SPILL_CAP * sizeof(uint32_t);
+    return (size_t)sm_count * 32 * 3 * SPILL_CAP * sizeof(uint32_t);   // up to 32 resident warps per SM
 }
 
 cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out, uint64_t n_active,

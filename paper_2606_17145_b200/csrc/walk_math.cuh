@@ -57,6 +57,14 @@ __device__ __forceinline__ float og_ex2(float x)
     return y;
 }
 
+// rsqrt.approx without the denormal-range rescaling of rsqrtf (arguments here are >= 1e-20).
+__device__ __forceinline__ float og_rsqrt(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 __device__ __forceinline__ void og_split(float r, float r2, const WalkConst &c, float &T, float &E)
 {
     const float w = r * c.k_w;
