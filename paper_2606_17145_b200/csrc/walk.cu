@@ -351,6 +351,7 @@ __device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, co
                                             const Target &t, const float hmax2g, const WalkConst &c, Accum &acc,
                                             const uint32_t lane, unsigned long long *cnt, LaneCount &lc)
 {
+    uint32_t it = 0u;
     for (;;) {
         if (lp.cur == 0u && lp.nxt < head) {
             const uint32_t sl = lp.nxt & (GW_NSEG - 1);
@@ -412,8 +413,10 @@ __device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, co
                 lc.ain += (k0 != 0) + (k1 != 0);
             }
         }
-        const uint32_t done = __reduce_min_sync(0xffffffffu, (cur == 0u) ? lp.nxt : lp.nxt - 1u);
-        if (done >= target) return done;
+        if ((++it & 1u) == 0u) {   // the exit test (a warp reduction) every second iteration
+            const uint32_t done = __reduce_min_sync(0xffffffffu, (cur == 0u) ? lp.nxt : lp.nxt - 1u);
+            if (done >= target) return done;
+        }
     }
 }
 
@@ -580,25 +583,41 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     const bool xwrap = (bX & bW) != 0u;
                     uint32_t openw = 0u, sloww = 0u;
                     uint32_t rem = bX;
-                    while (rem) {
-                        const int j = __ffs(rem) - 1;
+                    while (rem) {   // two staged nodes per iteration (independent chains)
+                        const int j0 = __ffs(rem) - 1;
                         rem &= rem - 1u;
-                        const float4 s = w.xn_com[j];
-                        const float4 x = w.xn_aux[j];
-                        float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
-                        if (xwrap) { dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c); }
-                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        const float rhs = GEOM ? c.theta2 * r2 : t.A * r2 * r2;
-                        const float diff = x.x - rhs;
-                        const bool inm = (Mt >> j) & 1u;
-                        const bool cand = inm && !(r2 > x.z);
-                        const bool fopen = diff > x.w;
-                        const bool facc = diff < -x.w && r2 > fmaxf(x.y, hi2m);
-                        const uint32_t bit = 1u << j;
-                        if (cand && fopen) openw |= bit;
-                        if (cand && !fopen && facc && r2 < c.rcut2_hi) accw |= bit;
-                        if (cand && !fopen && !facc) sloww |= bit;
-                        if (COUNT) { if (inm && !cand) ++lc.cull; if (cand && (fopen || facc)) ++lc.full; }
+                        const bool two = rem != 0u;
+                        const int j1 = two ? __ffs(rem) - 1 : j0;
+                        rem &= rem - 1u;
+                        const float4 s0 = w.xn_com[j0], s1 = w.xn_com[j1];
+                        const float4 x0 = w.xn_aux[j0], x1 = w.xn_aux[j1];
+                        float dx0 = s0.x - t.x, dy0 = s0.y - t.y, dz0 = s0.z - t.z;
+                        float dx1 = s1.x - t.x, dy1 = s1.y - t.y, dz1 = s1.z - t.z;
+                        if (xwrap) {
+                            dx0 = og_wrap(dx0, c); dy0 = og_wrap(dy0, c); dz0 = og_wrap(dz0, c);
+                            dx1 = og_wrap(dx1, c); dy1 = og_wrap(dy1, c); dz1 = og_wrap(dz1, c);
+                        }
+                        const float r20 = fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0));
+                        const float r21 = fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1));
+                        const float diff0 = x0.x - (GEOM ? c.theta2 * r20 : t.A * r20 * r20);
+                        const float diff1 = x1.x - (GEOM ? c.theta2 * r21 : t.A * r21 * r21);
+                        const uint32_t bit0 = 1u << j0, bit1 = two ? (1u << j1) : 0u;
+                        const bool cand0 = (Mt & bit0) && !(r20 > x0.z), cand1 = (Mt & bit1) && !(r21 > x1.z);
+                        const bool fopen0 = diff0 > x0.w, fopen1 = diff1 > x1.w;
+                        const bool facc0 = diff0 < -x0.w && r20 > fmaxf(x0.y, hi2m);
+                        const bool facc1 = diff1 < -x1.w && r21 > fmaxf(x1.y, hi2m);
+                        if (cand0 && fopen0) openw |= bit0;
+                        if (cand1 && fopen1) openw |= bit1;
+                        if (cand0 && !fopen0 && facc0 && r20 < c.rcut2_hi) accw |= bit0;
+                        if (cand1 && !fopen1 && facc1 && r21 < c.rcut2_hi) accw |= bit1;
+                        if (cand0 && !fopen0 && !facc0) sloww |= bit0;
+                        if (cand1 && !fopen1 && !facc1) sloww |= bit1;
+                        if (COUNT) {
+                            if ((Mt & bit0) && !cand0) ++lc.cull;
+                            if ((Mt & bit1) && !cand1) ++lc.cull;
+                            if (cand0 && (fopen0 || facc0)) ++lc.full;
+                            if (cand1 && (fopen1 || facc1)) ++lc.full;
+                        }
                     }
                     while (sloww) {   // per lane, rare
                         const int j = __ffs(sloww) - 1;

@@ -2,8 +2,8 @@
 (all targets active / the config's active subset, leaf_max = 8, potential on), checked on sampled
 outputs the oracle computes one by one, plus properties that hold at any size.
 
-Config 5 (512^3) needs ~25 GB of device memory and minutes of oracle time: it runs only with
-OG_TEST_HUGE=1."""
+Config 5 (512^3, both runs) needs ~25 GB of device memory, ~20 GB of host memory and ~75 s per run
+(measured on the B200 box); set OG_SKIP_HUGE=1 to leave it out."""
 import os
 
 import numpy as np
@@ -96,7 +96,7 @@ def test_full_size_sampled(B, name):
     _full_case(B, name)
 
 
-@pytest.mark.skipif(os.environ.get("OG_TEST_HUGE") != "1", reason="512^3: set OG_TEST_HUGE=1 (25 GB device, minutes of oracle)")
+@pytest.mark.skipif(os.environ.get("OG_SKIP_HUGE") == "1", reason="512^3 left out by OG_SKIP_HUGE=1")
 @pytest.mark.parametrize("name", ["nfw512", "nfw512_active10"])
 def test_full_size_sampled_huge(B, name):
     _full_case(B, name, nsample=1 << 13)
