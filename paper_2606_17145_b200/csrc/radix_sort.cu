@@ -18,6 +18,21 @@ constexpr int SORT_WARP_TILE = 32 * SORT_ITEMS;      // 512 consecutive keys per
 constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS; // 4096 keys per block
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
+// Lanes of the warp whose 8-bit digit equals this lane's (and whose `ok` flag equals this lane's): nine
+// ballots instead of __match_any_sync, which the hardware serialises over the distinct values.
+__device__ __forceinline__ uint32_t digit_peers(uint32_t d, bool ok)
+{
+    uint32_t peers = __ballot_sync(0xffffffffu, ok);
+    peers = ok ? peers : ~peers;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        const bool bit = (d >> b) & 1u;
+        const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+        peers &= bit ? bal : ~bal;
+    }
+    return peers;
+}
+
 __device__ __forceinline__ uint32_t lanemask_lt()
 {
     uint32_t m;
@@ -37,11 +52,12 @@ k_sort_hist(const uint64_t *__restrict__ keys, uint64_t n, int shift, uint32_t n
 #pragma unroll
     for (int r = 0; r < SORT_ITEMS; ++r) {
         const uint64_t i = base + (uint64_t)r * 32;
-        if (i < n) {
-            const uint32_t d = (uint32_t)(__ldg(keys + i) >> shift) & 255u;
+        {
+            const bool ok = i < n;
+            const uint32_t d = ok ? ((uint32_t)(__ldg(keys + i) >> shift) & 255u) : 0u;
             // aggregate equal digits inside the warp before touching shared memory
-            const uint32_t peers = __match_any_sync(__activemask(), d);
-            if ((peers & lanemask_lt()) == 0) atomicAdd(&h[d], __popc(peers));
+            const uint32_t peers = digit_peers(d, ok);
+            if (ok && (peers & lanemask_lt()) == 0) atomicAdd(&h[d], __popc(peers));
         }
     }
     __syncthreads();
@@ -93,20 +109,34 @@ k_sort_scan(uint32_t *__restrict__ hist, const uint32_t *__restrict__ ghist, uin
     }
 }
 
+// Stable scatter of one 4096-pair tile.  Every key is ranked inside the tile in input order (warp
+// match-any ranking, per-warp digit counters, exclusive prefix over the warps and over the digits),
+// the tile is reordered by digit in shared memory, and then written out: consecutive threads write
+// consecutive elements of a digit's run, so the global stores are coalesced runs instead of 32
+// scattered 8-byte writes per warp instruction.
+struct ScatterSmem {
+    uint64_t keys[SORT_TILE];
+    uint32_t vals[SORT_TILE];
+    uint32_t cnt[SORT_WARPS][256];
+    uint32_t gbase[256];    // global offset of the tile's first key of digit d, minus its position in the tile
+};
+
 __global__ void __launch_bounds__(SORT_THREADS)
 k_sort_scatter(const uint64_t *__restrict__ keys_in, const uint32_t *__restrict__ vals_in,
                uint64_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out, uint64_t n,
                int shift, uint32_t n_tiles, const uint32_t *__restrict__ offs)
 {
-    __shared__ uint32_t cnt[SORT_WARPS][256];
-    __shared__ uint32_t gbase[256];
+    extern __shared__ __align__(16) unsigned char sort_smem_raw[];
+    ScatterSmem &sm = *reinterpret_cast<ScatterSmem *>(sort_smem_raw);
+    __shared__ uint32_t wsum[SORT_WARPS];
     const uint32_t tid = threadIdx.x, lane = tid & 31u, wid = tid >> 5;
 #pragma unroll
-    for (int w = 0; w < SORT_WARPS; ++w) cnt[w][tid] = 0;
-    gbase[tid] = offs[(uint64_t)tid * n_tiles + blockIdx.x];
+    for (int w = 0; w < SORT_WARPS; ++w) sm.cnt[w][tid] = 0;
+    const uint32_t goff = offs[(uint64_t)tid * n_tiles + blockIdx.x];
     __syncthreads();
 
-    const uint64_t base = (uint64_t)blockIdx.x * SORT_TILE + wid * SORT_WARP_TILE + lane;
+    const uint64_t tile0 = (uint64_t)blockIdx.x * SORT_TILE;
+    const uint64_t base = tile0 + wid * SORT_WARP_TILE + lane;
     uint64_t key[SORT_ITEMS];
     uint32_t val[SORT_ITEMS];
     uint32_t rank[SORT_ITEMS];
@@ -122,37 +152,64 @@ k_sort_scatter(const uint64_t *__restrict__ keys_in, const uint32_t *__restrict_
 #pragma unroll
     for (int r = 0; r < SORT_ITEMS; ++r) {
         const bool ok = (base + (uint64_t)r * 32) < n;
-        const uint32_t d = ok ? ((uint32_t)(key[r] >> shift) & 255u) : 256u;
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        const uint32_t d = ok ? ((uint32_t)(key[r] >> shift) & 255u) : 0u;
+        const uint32_t peers = digit_peers(d, ok);
         const int leader = __ffs(peers) - 1;
         uint32_t b = 0;
         if ((int)lane == leader && ok) {
-            b = cnt[wid][d];
-            cnt[wid][d] = b + __popc(peers);
+            b = sm.cnt[wid][d];
+            sm.cnt[wid][d] = b + __popc(peers);
         }
         b = __shfl_sync(0xffffffffu, b, leader);
         rank[r] = b + __popc(peers & lt);
         __syncwarp();
     }
     __syncthreads();
-    // exclusive prefix over the warps of the tile, per digit
+    // per digit (thread tid = digit): exclusive prefix over the warps, then over the digits of the tile
+    uint32_t total = 0;
     {
-        uint32_t run = 0;
 #pragma unroll
         for (int w = 0; w < SORT_WARPS; ++w) {
-            const uint32_t c = cnt[w][tid];
-            cnt[w][tid] = run;
-            run += c;
+            const uint32_t c = sm.cnt[w][tid];
+            sm.cnt[w][tid] = total;
+            total += c;
         }
     }
+    uint32_t incl = total;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= (uint32_t)o) incl += y;
+    }
+    if (lane == 31) wsum[wid] = incl;
     __syncthreads();
+    uint32_t dstart = incl - total;   // first position of digit tid inside the tile
+#pragma unroll
+    for (int w = 0; w < SORT_WARPS; ++w) dstart += (w < (int)wid) ? wsum[w] : 0u;
+#pragma unroll
+    for (int w = 0; w < SORT_WARPS; ++w) sm.cnt[w][tid] += dstart;
+    sm.gbase[tid] = goff - dstart;
+    __syncthreads();
+    // reorder the tile by digit in shared memory
 #pragma unroll
     for (int r = 0; r < SORT_ITEMS; ++r) {
         if ((base + (uint64_t)r * 32) < n) {
             const uint32_t d = (uint32_t)(key[r] >> shift) & 255u;
-            const uint32_t p = gbase[d] + cnt[wid][d] + rank[r];
-            keys_out[p] = key[r];
-            vals_out[p] = val[r];
+            const uint32_t p = sm.cnt[wid][d] + rank[r];
+            sm.keys[p] = key[r];
+            sm.vals[p] = val[r];
+        }
+    }
+    __syncthreads();
+    const uint32_t in_tile = (uint32_t)min((uint64_t)SORT_TILE, n - tile0);
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        const uint32_t i = tid + r * SORT_THREADS;
+        if (i < in_tile) {
+            const uint64_t k = sm.keys[i];
+            const uint32_t p = sm.gbase[(uint32_t)(k >> shift) & 255u] + i;
+            keys_out[p] = k;
+            vals_out[p] = sm.vals[i];
         }
     }
 }
@@ -175,7 +232,9 @@ cudaError_t ogk_radix_sort(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, u
     uint32_t *hist = reinterpret_cast<uint32_t *>(scratch);
     uint32_t *ghist = hist + (size_t)n_tiles * 256;
     const int passes = (end_bit - begin_bit + 7) / 8;
-    cudaError_t e = cudaMemsetAsync(ghist, 0, 8 * 256 * sizeof(uint32_t), st);
+    cudaError_t e = cudaFuncSetAttribute(k_sort_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem));
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(ghist, 0, 8 * 256 * sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
     uint64_t *kin = keys, *kout = keys_alt;
     uint32_t *vin = vals, *vout = vals_alt;
@@ -183,7 +242,7 @@ cudaError_t ogk_radix_sort(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, u
         const int shift = begin_bit + 8 * p;
         k_sort_hist<<<n_tiles, SORT_THREADS, 0, st>>>(kin, n, shift, n_tiles, hist, ghist + 256 * p);
         k_sort_scan<<<256, 1024, 0, st>>>(hist, ghist + 256 * p, n_tiles);
-        k_sort_scatter<<<n_tiles, SORT_THREADS, 0, st>>>(kin, vin, kout, vout, n, shift, n_tiles, hist);
+        k_sort_scatter<<<n_tiles, SORT_THREADS, sizeof(ScatterSmem), st>>>(kin, vin, kout, vout, n, shift, n_tiles, hist);
         uint64_t *tk = kin; kin = kout; kout = tk;
         uint32_t *tv = vin; vin = vout; vout = tv;
     }

@@ -473,6 +473,9 @@ k_walk_group(const __grid_constant__ WalkArgs a)
         const float hi2m = hi2 * (1.0f + OG_GM);   // own softening guard threshold (R16), padded
         Accum acc = {0.f, 0.f, 0.f, 0.f};
         LaneCount lc = {0, 0, 0, 0, 0, 0};
+        // diag (OG_COUNT): groups binned by their largest half extent relative to r_cut
+        uint32_t dg_gen = 0, dg_bat = 0;
+        const long long dg_t0 = COUNT ? clock64() : 0;
         int top = 0, pl_top = 0;
         uint32_t pl_items = 0, spill_n = 0;
         uint32_t head = 0, tail = 0;          // ring: segments produced / finished by all lanes
@@ -547,23 +550,12 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 const uint32_t Mt = transpose32((cls >= CL_ACCEPT) ? imask : 0u, lane);
                 __syncwarp();
                 if (COUNT) {   // group-level outcomes counted as the per-target visits they stand for
-                    if (cls >= CL_ACCEPT && imask) {   // diag: lane-slots a team-granular evaluation would need
-                        const int o = (cls == CL_ACCEPT) ? 16 : 24;
-                        int n4 = 0, n8 = 0, n16 = 0;
-                        for (int q = 0; q < 8; ++q) n4 += ((imask >> (4 * q)) & 0xfu) != 0;
-                        for (int q = 0; q < 4; ++q) n8 += ((imask >> (8 * q)) & 0xffu) != 0;
-                        for (int q = 0; q < 2; ++q) n16 += ((imask >> (16 * q)) & 0xffffu) != 0;
-                        atomicAdd(&a.counters[OGC_DIAG0 + o + 0], (unsigned long long)__popc(imask));
-                        atomicAdd(&a.counters[OGC_DIAG0 + o + 1], (unsigned long long)(4 * n4));
-                        atomicAdd(&a.counters[OGC_DIAG0 + o + 2], (unsigned long long)(8 * n8));
-                        atomicAdd(&a.counters[OGC_DIAG0 + o + 3], (unsigned long long)(16 * n16));
-                        atomicAdd(&a.counters[OGC_DIAG0 + o + 4], 32ull);
-                    }
                     const uint32_t bO = __ballot_sync(0xffffffffu, cls == CL_OPEN);
                     if (lane == 0) {
                         atomicAdd(&a.counters[OGC_CL_OPEN], (unsigned long long)__popc(bO));
                         atomicAdd(&a.counters[OGC_CL_ACCEPT], (unsigned long long)__popc(bA));
                         atomicAdd(&a.counters[OGC_CL_GENERIC], (unsigned long long)__popc(bX));
+                        dg_gen += __popc(bX); ++dg_bat;
                         atomicAdd(&a.counters[OGC_CL_DROP], (unsigned long long)(total - __popc(bA | bX | bO)));
                         atomicAdd(&a.counters[OGC_BATCHES], 1ull);
                     }
@@ -764,6 +756,15 @@ k_walk_group(const __grid_constant__ WalkArgs a)
             a.acc_out[3 * (size_t)out + 1] = acc.ay;
             a.acc_out[3 * (size_t)out + 2] = acc.az;
             if (POT) a.pot_out[out] = acc.pot;
+        }
+        if (COUNT && lane == 0) {
+            const float e = fmaxf(g.ghx, fmaxf(g.ghy, g.ghz)) / c.rcut;
+            const int b = e < 0.025f ? 0 : e < 0.05f ? 1 : e < 0.1f ? 2 : e < 0.2f ? 3 : e < 0.4f ? 4 : 5;
+            atomicAdd(&a.counters[OGC_DIAG0 + b], 1ull);
+            atomicAdd(&a.counters[OGC_DIAG0 + 6 + b], (unsigned long long)(clock64() - dg_t0));
+            atomicAdd(&a.counters[OGC_DIAG0 + 12 + b], (unsigned long long)dg_gen);
+            atomicAdd(&a.counters[OGC_DIAG0 + 18 + b], (unsigned long long)head);
+            atomicAdd(&a.counters[OGC_DIAG0 + 24 + b], (unsigned long long)(lc.ain + lc.pin));
         }
         if (COUNT) {
             const uint32_t v[6] = {lc.full, lc.cull, lc.ain, lc.pin, lc.psoft, lc.pout};
