@@ -139,7 +139,7 @@ og_tree *og_tree_build(const float *pos, const float *mass, const float *soft, u
  *              required; NULL -> all n particles in identity order (n_active must be n)
  *   a_old      DEVICE f32 [n_active] |a| of the previous step in active order (R23);
  *              NULL -> geometric criterion l^2 > theta^2 r^2 (R22)
- *   acc_out    DEVICE f32 [n_active][3], overwritten
+ *   acc_out    DEVICE f32 [n_active][3], overwritten (n_active == 0: nothing is done, OG_OK)
  *   pot_out    DEVICE f32 [n_active], overwritten, or NULL
  * Returns OG_OK or a negative og_status (also a previously latched device condition).
  */

@@ -241,6 +241,7 @@ extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx,
 {
     g_err[0] = 0;
     if (!t) { og_set_error("tree is NULL"); return OG_ERR_INVALID_ARG; }
+    if (n_active == 0) return OG_OK;   // empty active list: nothing to do (pointers of empty buffers may be NULL)
     if (!acc_out) { og_set_error("acc_out is NULL"); return OG_ERR_INVALID_ARG; }
     if (!active_idx && n_active != t->n) {
         og_set_error("active_idx == NULL requires n_active == n (%llu != %llu)", (unsigned long long)n_active,
@@ -248,7 +249,6 @@ extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx,
         return OG_ERR_INVALID_ARG;
     }
     if (n_active >= (1ull << 31)) { og_set_error("n_active out of range"); return OG_ERR_INVALID_ARG; }
-    if (n_active == 0) return OG_OK;
     cudaStream_t st = (cudaStream_t)stream;
     t->last_stream = st;
     if (!active_idx) {

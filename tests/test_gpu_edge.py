@@ -1,0 +1,175 @@
+"""-m gpu: edge and degenerate cases of the path through the C ABI, each against the oracle
+(or its closed form): tiny and ragged sizes, coincident particles, deep single-child chains and the
+node-capacity latch, groups that straddle the periodic wall (per-lane nearest-image path), targets with
+a_old = 0, arbitrary / duplicated / empty / invalid active lists, caller-supplied workspace, the
+HOST-buffer entry point, position validation."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_17145_b200 import workloads as W
+from gpu_common import check_acc, rel_err_scalar
+
+pytestmark = pytest.mark.gpu
+
+L, RS = 1.0, 1.25 / 64
+EPS = 0.02 / 32
+
+
+@pytest.fixture(scope="module")
+def B(cuda_device):
+    from paper_2606_17145_b200 import binding
+    return binding
+
+
+def _wl(pos, mass=None, eps=None, L=L, r_s=RS, alpha=0.005):
+    pos = np.ascontiguousarray(pos, np.float32)
+    n = pos.shape[0]
+    mass = np.full(n, 1.0 / max(n, 1), np.float32) if mass is None else np.asarray(mass, np.float32)
+    eps = np.full(n, EPS, np.float32) if eps is None else np.asarray(eps, np.float32)
+    return W.Workload("edge", pos, mass, eps, L, r_s, alpha=alpha)
+
+
+def _both(B, w, active=None, a_old=None, leaf_max=8, flags=0, max_nodes=0):
+    """GPU and oracle results for the same inputs -> (acc_gpu, pot_gpu, acc_orc, pot_orc)."""
+    import torch
+    prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=leaf_max,
+                        max_nodes=max_nodes, flags=B.OG_PERIODIC | flags)
+    pos, mass, eps = (torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps))
+    tree = B.og_tree_build(pos, mass, eps, w.L, prm)
+    act = None if active is None else torch.from_numpy(np.asarray(active, np.uint32).view(np.int32)).cuda()
+    ao = None if a_old is None else torch.from_numpy(np.asarray(a_old, np.float32)).cuda()
+    a, p = B.og_shortrange_accel(tree, act, ao)
+    assert B.og_tree_status(tree) == B.OG_OK, B.og_last_error()
+    oprm = oracle.make_params(w.L, w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta,
+                              leaf_max=leaf_max)
+    ot = oracle.build_tree(w.pos, w.mass, w.eps, oprm)
+    assert B.og_tree_stats(tree)["n_nodes"] == ot.n_nodes
+    ao_, po_, _ = oracle.walk(ot, None if active is None else np.asarray(active, np.uint32),
+                              None if a_old is None else np.asarray(a_old, np.float32), want_counters=False)
+    B.og_tree_free(tree)
+    return a.cpu().numpy(), p.cpu().numpy(), ao_, po_
+
+
+def test_single_particle(B):
+    a, p, ao, po = _both(B, _wl([[0.3, 0.4, 0.5]]))
+    assert np.all(a == 0) and np.all(p == 0) and np.all(ao == 0)
+
+
+def test_two_coincident_particles(B):
+    """C5: distinct coincident particles: force 0, potential -(14/5) G m / h."""
+    w = _wl([[0.5, 0.5, 0.5], [0.5, 0.5, 0.5]])
+    a, p, ao, po = _both(B, w)
+    h = np.float32(2.8) * np.float32(EPS)
+    assert np.all(a == 0) and np.all(ao == 0)
+    assert np.allclose(p, -2.8 * 0.5 / h, rtol=1e-6) and np.allclose(po, -2.8 * 0.5 / float(h), rtol=1e-6)
+
+
+@pytest.mark.parametrize("n", [2, 9, 31, 32, 33, 65, 1000])
+def test_ragged_sizes(B, n):
+    rng = np.random.default_rng(n)
+    c = rng.random(3) * 0.8 + 0.1
+    pos = np.mod(c + 0.02 * rng.standard_normal((n, 3)), 1.0)
+    a, p, ao, po = _both(B, _wl(pos))
+    check_acc(a, ao, what=f"n={n}")
+    ep = rel_err_scalar(p, po)
+    assert ep.size == 0 or ep.max() <= 1e-4
+
+
+def test_group_straddles_periodic_wall(B):
+    """A tight cluster cut by the faces x = 0 / L in all three axes: Morton-consecutive targets sit on both
+    sides of the wall, so sources cannot be pre-shifted for the whole group (per-lane nearest-image path)."""
+    rng = np.random.default_rng(5)
+    pos = np.mod(0.015 * rng.standard_normal((4000, 3)), 1.0)
+    w = _wl(pos)
+    a1, p1, ao1, po1 = _both(B, w)
+    check_acc(a1, ao1, what="wall geometric")
+    a_old = np.linalg.norm(ao1, axis=1).astype(np.float32)
+    a2, p2, ao2, po2 = _both(B, w, a_old=a_old)
+    check_acc(a2, ao2, what="wall relative")
+    ep = rel_err_scalar(p2, po2)
+    assert np.percentile(ep, 99) <= 1e-4 and ep.max() <= 1e-2
+
+
+def test_deep_chain_and_node_overflow_latch(B):
+    """Near-coincident particles create single-child chains down to level 21 (R6); a too small node
+    capacity latches OG_ERR_NODE_OVERFLOW instead of writing out of bounds."""
+    import torch
+    rng = np.random.default_rng(11)
+    base = np.array([0.123456, 0.654321, 0.333333])
+    pos = np.concatenate([base + 3e-7 * rng.random((64, 3)), rng.random((200, 3))])
+    w = _wl(pos)
+    a, p, ao, po = _both(B, w, leaf_max=1, max_nodes=4096)
+    check_acc(a, ao, what="deep chain")
+    prm = B.make_params(w.r_s, leaf_max=1, max_nodes=64)
+    t = B.og_tree_build(*(torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps)), w.L, prm)
+    assert B.og_tree_status(t) == B.OG_ERR_NODE_OVERFLOW
+    assert "status" in B.og_last_error()
+    B.og_tree_free(t)
+
+
+def test_a_old_zero_opens_everything(B):
+    """A = 0 => G M l^2 > 0 always opens (R14): those targets get the direct sum within r_cut."""
+    w = W.make("uniform32", small=True)
+    a_old = np.zeros(w.n, np.float32)
+    a_old[::2] = 1.0
+    a, p, ao, po = _both(B, w, a_old=a_old)
+    check_acc(a, ao, what="a_old mixed zero")
+    ad, _ = oracle.direct(w.pos, w.mass, w.eps, oracle.make_params(w.L, w.r_s))
+    check_acc(a[1::2], ad[1::2], p99=2e-5, mx=1e-3, what="a_old=0 vs direct")
+
+
+def test_active_lists(B):
+    """Arbitrary order, duplicates, a single target, and the empty list."""
+    import torch
+    w = W.make("nfw256", small=True)
+    rng = np.random.default_rng(3)
+    act = rng.permutation(w.n)[:777].astype(np.uint32)
+    act[10] = act[500]                      # duplicate
+    a, p, ao, po = _both(B, w, active=act)
+    check_acc(a, ao, what="active subset")
+    assert np.array_equal(a[10], a[500])
+    a1, p1, ao1, po1 = _both(B, w, active=act[:1])
+    check_acc(a1, ao1, what="one target")
+    prm = B.make_params(w.r_s)
+    t = B.og_tree_build(*(torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps)), w.L, prm)
+    empty = torch.empty(0, dtype=torch.int32, device="cuda")
+    out = torch.empty((0, 3), dtype=torch.float32, device="cuda")
+    B.og_shortrange_accel(t, empty, None, acc_out=out, want_pot=False)
+    assert B.og_tree_status(t) == B.OG_OK
+    bad = torch.tensor([0, w.n + 5], dtype=torch.int32, device="cuda")     # out of range -> latched
+    B.og_shortrange_accel(t, bad, None)
+    assert B.og_tree_status(t) == B.OG_ERR_INVALID_ARG
+    B.og_tree_free(t)
+
+
+def test_workspace_validate_and_host_entry(B):
+    import torch
+    w = W.make("lattice128", small=True)
+    prm = B.make_params(w.r_s, alpha=w.alpha, flags=B.OG_PERIODIC | B.OG_VALIDATE_POS)
+    pos, mass, eps = (torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps))
+    ws = torch.empty(B.og_tree_workspace_bytes(w.n, prm) + 256, dtype=torch.uint8, device="cuda")
+    off = (-ws.data_ptr()) % 256
+    t = B.og_tree_build(pos, mass, eps, w.L, prm, workspace=ws[off:])
+    a_ws, p_ws = B.og_shortrange_accel(t, None, None)
+    assert B.og_tree_status(t) == B.OG_OK
+    t2 = B.og_tree_build(pos, mass, eps, w.L, prm)
+    a_pool, p_pool = B.og_shortrange_accel(t2, None, None)
+    assert torch.equal(a_ws, a_pool) and torch.equal(p_ws, p_pool)
+    with pytest.raises(B.OgError):
+        B.og_tree_build(pos, mass, eps, w.L, prm, workspace=ws[off:off + 4096])
+    # HOST-buffer entry point = the two device calls
+    a_h, p_h = B.og_shortrange_accel_host(torch.from_numpy(w.pos), torch.from_numpy(w.mass), torch.from_numpy(w.eps),
+                                          w.L, prm)
+    assert torch.equal(a_h, a_pool.cpu()) and torch.equal(p_h, p_pool.cpu())
+    # pot_out = NULL gives the same accelerations
+    a_np, none = B.og_shortrange_accel(t2, None, None, want_pot=False)
+    assert none is None and torch.equal(a_np, a_pool)
+    B.og_tree_free(t)
+    B.og_tree_free(t2)
+    # position outside [0, box) is latched when OG_VALIDATE_POS is set
+    badpos = pos.clone()
+    badpos[7, 1] = w.L
+    t3 = B.og_tree_build(badpos, mass, eps, w.L, prm)
+    assert B.og_tree_status(t3) == B.OG_ERR_BAD_POSITION
+    B.og_tree_free(t3)
