@@ -13,7 +13,7 @@ namespace {
 
 constexpr int SORT_THREADS = 256;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
-constexpr int SORT_ITEMS = 16;                       // keys per thread
+constexpr int SORT_ITEMS = 8;                        // keys per thread
 constexpr int SORT_WARP_TILE = 32 * SORT_ITEMS;      // 512 consecutive keys per warp
 constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS; // 4096 keys per block
 
