@@ -264,7 +264,10 @@ __device__ __forceinline__ int classify_node(const float4 n0, float R, float ng,
         rhs_min = c.alpha * g.amin * rmin2 * rmin2;
     }
     if (lhs > rhs_max * (1.0f + OG_GM)) return CL_OPEN;
-    shifted = fmaxf(fx, fmaxf(fy, fz)) < 0.5f * c.L * (1.0f - OG_GM) && fminf(kx, fminf(ky, kz)) >= 0.0f;
+    // x - k L is exact for k = 0 and, by Sterbenz, for k = 1 with x >= L/2
+    const float hL = 0.5f * c.L;
+    shifted = fmaxf(fx, fmaxf(fy, fz)) < hL * (1.0f - OG_GM) && (kx == 0.0f || (kx == 1.0f && n0.x >= hL)) &&
+              (ky == 0.0f || (ky == 1.0f && n0.y >= hL)) && (kz == 0.0f || (kz == 1.0f && n0.z >= hL));
     if (shifted) sc = make_float4(fmaf(-c.L, kx, n0.x), fmaf(-c.L, ky, n0.y), fmaf(-c.L, kz, n0.z), GM);
     else sc = make_float4(n0.x, n0.y, n0.z, GM);
     const float ng2 = ng * ng;
@@ -297,7 +300,9 @@ __device__ __forceinline__ int classify_particle(float4 &p, const GroupInfo &g, 
     const float nx = fmaxf(adx - g.ghx, 0.f), ny = fmaxf(ady - g.ghy, 0.f), nz = fmaxf(adz - g.ghz, 0.f);
     if (fmaf(nz, nz, fmaf(ny, ny, nx * nx)) > c.rcut2 * (1.0f + OG_GM)) return 0;
     const float halfL = 0.5f * c.L * (1.0f - OG_GM);
-    if (fmaxf(adx + g.ghx, fmaxf(ady + g.ghy, adz + g.ghz)) < halfL && fminf(kx, fminf(ky, kz)) >= 0.0f) {
+    const float hL = 0.5f * c.L;
+    if (fmaxf(adx + g.ghx, fmaxf(ady + g.ghy, adz + g.ghz)) < halfL && (kx == 0.0f || (kx == 1.0f && p.x >= hL)) &&
+        (ky == 0.0f || (ky == 1.0f && p.y >= hL)) && (kz == 0.0f || (kz == 1.0f && p.z >= hL))) {
         p.x = fmaf(-c.L, kx, p.x); p.y = fmaf(-c.L, ky, p.y); p.z = fmaf(-c.L, kz, p.z);
         return 1;
     }
@@ -466,6 +471,14 @@ k_walk_group(const __grid_constant__ WalkArgs a)
             g.amin = warp_min_pos(fabsf(t.aold)); g.amax = warp_max_pos(fabsf(t.aold));
             const float hm = warp_max_pos(t.h);
             g.hmax2 = hm * hm;
+            // A group that lies entirely in the upper quarter of the box along an axis is moved to the image
+            // x - L (exact: L/2 <= x < L): its sources across the upper face then need no shift and the
+            // others a shift by -L, which is exact for a source in the upper half (classify_node), so groups
+            // next to the upper faces pre-shift their sources like all others.
+            const float halfL = 0.75f * c.L;
+            if (lox >= halfL) { t.x -= c.L; g.gcx = 0.5f * ((lox - c.L) + (hix - c.L)); }
+            if (loy >= halfL) { t.y -= c.L; g.gcy = 0.5f * ((loy - c.L) + (hiy - c.L)); }
+            if (loz >= halfL) { t.z -= c.L; g.gcz = 0.5f * ((loz - c.L) + (hiz - c.L)); }
         }
         // lanes whose target is the same sorted slot (duplicates in active_idx; the mirrored tail lanes)
         const uint32_t peers = __match_any_sync(0xffffffffu, t.slot);
