@@ -163,6 +163,12 @@ struct __align__(16) WarpSmem {
     uint32_t pl_start[GW_PLIST], pl_cnt[GW_PLIST], pl_mask[GW_PLIST];
 };
 
+// w |= bit if p, as one predicated instruction (the compiler's select + or costs two)
+__device__ __forceinline__ void or_if(uint32_t &w, const uint32_t bit, const bool p)
+{
+    asm("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %2, 0;\n\t@q or.b32 %0, %0, %1;\n\t}" : "+r"(w) : "r"(bit), "r"((uint32_t)p));
+}
+
 __device__ __forceinline__ uint32_t lanemask_lt()
 {
     uint32_t m;
@@ -611,12 +617,12 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                         const bool fopen0 = diff0 > x0.w, fopen1 = diff1 > x1.w;
                         const bool facc0 = diff0 < -x0.w && r20 > fmaxf(x0.y, hi2m);
                         const bool facc1 = diff1 < -x1.w && r21 > fmaxf(x1.y, hi2m);
-                        if (cand0 && fopen0) openw |= bit0;
-                        if (cand1 && fopen1) openw |= bit1;
-                        if (cand0 && !fopen0 && facc0 && r20 < c.rcut2_hi) accw |= bit0;
-                        if (cand1 && !fopen1 && facc1 && r21 < c.rcut2_hi) accw |= bit1;
-                        if (cand0 && !fopen0 && !facc0) sloww |= bit0;
-                        if (cand1 && !fopen1 && !facc1) sloww |= bit1;
+                        or_if(openw, bit0, cand0 && fopen0);
+                        or_if(openw, bit1, cand1 && fopen1);
+                        or_if(accw, bit0, cand0 && !fopen0 && facc0 && r20 < c.rcut2_hi);
+                        or_if(accw, bit1, cand1 && !fopen1 && facc1 && r21 < c.rcut2_hi);
+                        or_if(sloww, bit0, cand0 && !fopen0 && !facc0);
+                        or_if(sloww, bit1, cand1 && !fopen1 && !facc1);
                         if (COUNT) {
                             if ((Mt & bit0) && !cand0) ++lc.cull;
                             if ((Mt & bit1) && !cand1) ++lc.cull;
