@@ -7,18 +7,19 @@
 // lane accepts / opens exactly the nodes its own serial walk would (C6): each pending entry
 // carries a 32-bit lane mask = the lanes that opened the parent.  Per iteration the warp pops
 // up to 32 child nodes from a shared-memory stack of (first, count, mask) ranges and lane k
-// loads node k (4 x LDG.128, children are contiguous) and classifies it against the GROUP
-// (bounding box of the 32 targets, range of a_old, largest h): dropped by the cutoff box,
-// opened by every target, accepted by every target, or undecided.  Only the last two classes
-// are staged in shared memory and scanned by all lanes (broadcast LDS.128): accepted-by-all
-// nodes cost one monopole per lane with no decision work, undecided ones get the exact
-// per-lane cull / opening test and a ballot yields the mask of the children.  Opened leaves go
-// to a second range list whose particles are staged (after a group-level cutoff test and an
-// exact periodic shift) in segments of 32.  Staged sources live in a shared-memory ring of GW_NSEG
-// segments; every lane walks the set bits of its OWN words W[seg][lane] and may lag up to a whole
-// ring behind the producer, so a lane idles only when it has nothing left in the ring.  The split
-// factors T, E are evaluated in registers (polynomial x ex2, walk_math.cuh).  Results are written
-// straight to the caller's order (a7 fused).
+// loads node k (3 x LDG.128 of the packed walk record, children are contiguous) and classifies
+// it against the GROUP (bounding box of the 32 targets, range of a_old, largest h): dropped by
+// the cutoff box, opened by every target, accepted by every target, or undecided.  Undecided
+// nodes are staged in shared memory and tested by all lanes, two per loop iteration (broadcast
+// LDS.128, branch-free; the rare lanes inside a guard region or within OG_BAND of a threshold take
+// the exact path); a 32 x 32 bit transpose of the per-lane "open" words yields the masks of the
+// children.  Accepted nodes and the particles of opened leaves (after a group-level cutoff test
+// and an exact periodic shift to the group's image) are staged in a shared-memory ring of GW_NSEG
+// segments of 32 sources; every lane walks the set bits of its OWN words W[seg][lane], two
+// sources per iteration, and may lag up to a whole ring behind the producer, so a lane idles
+// only when it has nothing left in the ring.  The split factors T, E are evaluated in registers
+// (polynomial x ex2, walk_math.cuh).  Results are written straight to the caller's order (a7
+// fused).  DESIGN.md Sec. 5 has the measured per-group counts and the instruction budget.
 //
 // k_walk_simple: one thread per target with a private stack; debugging / comparison only.
 #include "walk_math.cuh"
