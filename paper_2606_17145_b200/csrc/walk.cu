@@ -136,6 +136,9 @@ k_walk_simple(const __grid_constant__ WalkArgs a)
 #ifndef OG_GW_NSEG
 #define OG_GW_NSEG 8
 #endif
+#ifndef OG_GW_SPARSE_G
+#define OG_GW_SPARSE_G 8   // targets per warp for sparse active subsets (4, 8 or 16; zoom: 31.9 / 31.3 / 36.7 ms)
+#endif
 #ifndef OG_GW_STACK
 #define OG_GW_STACK 256
 #endif
@@ -432,16 +435,25 @@ __device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, co
     }
 }
 
-template <bool GEOM, bool POT, bool COUNT>
+// G = targets per warp (32, or 8 for sparse active subsets), K = 32 / G lanes per target: lane = s * G + t
+// serves target t and the staged sources / undecided nodes whose slot index is = s (mod K); all lane masks
+// (imask, children masks) are G-bit TARGET masks; the K partial sums of a target are added at the end.
+template <bool GEOM, bool POT, bool COUNT, int G>
 __global__ void __launch_bounds__(GW_THREADS, OG_GW_MINBLOCKS)
 k_walk_group(const __grid_constant__ WalkArgs a)
 {
+    constexpr int K = 32 / G;
+    constexpr uint32_t TMASK = (G == 32) ? 0xffffffffu : ((1u << (G & 31)) - 1u);           // the G targets
+    constexpr uint32_t REP = (G == 32) ? 1u : (G == 16) ? 0x00010001u : (G == 8) ? 0x01010101u : 0x11111111u;       // replicate a target mask to all slices
+    constexpr uint32_t SLICE0 = (G == 32) ? 0xffffffffu : (G == 16) ? 0x55555555u : (G == 8) ? 0x11111111u : 0x01010101u;  // slots = 0 (mod K)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WarpSmem *wsm = reinterpret_cast<WarpSmem *>(smem_raw);
     const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
     WarpSmem &w = wsm[wid];
     const uint32_t lt = lanemask_lt();
-    const uint32_t mybit = 1u << lane;
+    const uint32_t tl = lane & (G - 1), sl = lane / G;        // target and slice of this lane
+    const uint32_t mybit = 1u << tl;                          // in target masks
+    const uint32_t myslots = SLICE0 << sl;                    // the slots this lane evaluates
     const WalkConst &c = a.c;
     unsigned long long *cnt = COUNT ? a.counters : nullptr;
     uint32_t *sp_start = a.spill + (size_t)(blockIdx.x * GW_WARPS + wid) * 3 * a.spill_cap;
@@ -458,9 +470,9 @@ k_walk_group(const __grid_constant__ WalkArgs a)
         if (lane == 0) gi = atomicAdd(a.work, 1u);
         gi = __shfl_sync(0xffffffffu, gi, 0);
         if (gi >= a.n_groups) break;
-        const uint32_t k = gi * 32u + lane;
+        const uint32_t k = gi * (uint32_t)G + tl;
         const bool valid = k < a.n_active;
-        const uint32_t klast = min(gi * 32u + 31u, a.n_active - 1u);
+        const uint32_t klast = min(gi * (uint32_t)G + (uint32_t)(G - 1), a.n_active - 1u);
         uint32_t out = 0;
         // lanes past the end mirror the last target (keeps the group's bounds tight); they never
         // appear in a mask and write nothing
@@ -488,7 +500,7 @@ k_walk_group(const __grid_constant__ WalkArgs a)
             if (loz >= halfL) { t.z -= c.L; g.gcz = 0.5f * ((loz - c.L) + (hiz - c.L)); }
         }
         // lanes whose target is the same sorted slot (duplicates in active_idx; the mirrored tail lanes)
-        const uint32_t peers = __match_any_sync(0xffffffffu, t.slot);
+        const uint32_t peers = __match_any_sync(0xffffffffu, t.slot) & TMASK;   // as a target mask
         const float hi2 = t.h * t.h;
         const float hi2m = hi2 * (1.0f + OG_GM);   // own softening guard threshold (R16), padded
         Accum acc = {0.f, 0.f, 0.f, 0.f};
@@ -502,7 +514,7 @@ k_walk_group(const __grid_constant__ WalkArgs a)
         bool anywrap = false;                 // some staged source of this group is not pre-shifted
         LanePos lp = {0u, 0u, 0u, 0u};
         {
-            const uint32_t vm = __ballot_sync(0xffffffffu, valid);
+            const uint32_t vm = __ballot_sync(0xffffffffu, valid) & TMASK;
             if (lane == 0) { w.st_start[0] = 0; w.st_cnt[0] = 1; w.st_mask[0] = vm; }
             top = 1;
             __syncwarp();
@@ -567,7 +579,7 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 const uint32_t bW = __ballot_sync(0xffffffffu, cls >= CL_ACCEPT && !shifted);
                 anywrap |= bW != 0u;
                 // Mt: bit j = my target is in the mask of the node lane j holds
-                const uint32_t Mt = transpose32((cls >= CL_ACCEPT) ? imask : 0u, lane);
+                const uint32_t Mt = transpose32((cls >= CL_ACCEPT) ? imask * REP : 0u, lane);
                 __syncwarp();
                 if (COUNT) {   // group-level outcomes counted as the per-target visits they stand for
                     const uint32_t bO = __ballot_sync(0xffffffffu, cls == CL_OPEN);
@@ -582,8 +594,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     for (uint32_t j = 0; j < total; ++j) {
                         const uint32_t mj = __shfl_sync(0xffffffffu, imask, j);
                         const int cj = __shfl_sync(0xffffffffu, cls, j);
-                        if ((mj & mybit) && (cj == CL_OPEN || cj == CL_ACCEPT)) ++lc.full;
-                        if ((mj & mybit) && cj == CL_DROP) ++lc.cull;
+                        if (sl == 0u && (mj & mybit) && (cj == CL_OPEN || cj == CL_ACCEPT)) ++lc.full;
+                        if (sl == 0u && (mj & mybit) && cj == CL_DROP) ++lc.cull;
                     }
                 }
                 // Undecided nodes: every lane tests every staged node (broadcast LDS) branch-free on
@@ -594,9 +606,12 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 if (bX != 0u) {
                     const bool xwrap = (bX & bW) != 0u;
                     uint32_t openw = 0u, sloww = 0u;
-                    uint32_t rem = bX;
-                    while (rem) {   // two staged nodes per iteration (independent chains)
-                        const int j0 = __ffs(rem) - 1;
+                    // G = 32: every lane tests every node (uniform loop); G < 32: slice s of a target tests the
+                    // nodes of the slots = s (mod K), so K different nodes are tested per step
+                    uint32_t rem = bX & myslots;
+                    while (G == 32 ? (rem != 0u) : __any_sync(0xffffffffu, rem != 0u)) {   // two nodes per iteration
+                        const bool one = rem != 0u;
+                        const int j0 = (__ffs(rem) - 1) & 31;
                         rem &= rem - 1u;
                         const bool two = rem != 0u;
                         const int j1 = two ? __ffs(rem) - 1 : j0;
@@ -613,7 +628,7 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                         const float r21 = fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1));
                         const float diff0 = x0.x - (GEOM ? c.theta2 * r20 : t.A * r20 * r20);
                         const float diff1 = x1.x - (GEOM ? c.theta2 * r21 : t.A * r21 * r21);
-                        const uint32_t bit0 = 1u << j0, bit1 = two ? (1u << j1) : 0u;
+                        const uint32_t bit0 = (G == 32 || one) ? (1u << j0) : 0u, bit1 = two ? (1u << j1) : 0u;
                         const bool cand0 = (Mt & bit0) && !(r20 > x0.z), cand1 = (Mt & bit1) && !(r21 > x1.z);
                         const bool fopen0 = diff0 > x0.w, fopen1 = diff1 > x1.w;
                         const bool facc0 = diff0 < -x0.w && r20 > fmaxf(x0.y, hi2m);
@@ -667,9 +682,12 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     }
                     __syncwarp();
                     myopen = transpose32(openw, lane);   // lane j: the lanes that open the node lane j holds
+                    if (G == 16) myopen = (myopen | (myopen >> 16)) & TMASK;            // -> target mask
+                    if (G == 8) { myopen |= myopen >> 16; myopen = (myopen | (myopen >> 8)) & TMASK; }
+                    if (G == 4) { myopen |= myopen >> 16; myopen |= myopen >> 8; myopen = (myopen | (myopen >> 4)) & TMASK; }
                 }
                 if ((bA | bX) != 0u) {
-                    w.W[head & (GW_NSEG - 1)][lane] = (Mt & bA) | accw;
+                    w.W[head & (GW_NSEG - 1)][lane] = (Mt & bA & myslots) | accw;
                     if (COUNT && lane == 0) w.seg_flags[head & (GW_NSEG - 1)] = 0u;
                     ++head;
                 }
@@ -741,7 +759,7 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 {
                     int lo = 0;
 #pragma unroll
-                    for (int step = 16; step >= 1; step >>= 1) {
+                    for (int step = G / 2; step >= 1; step >>= 1) {   // lanes 0 .. G-1 hold the G targets
                         const uint32_t v = __shfl_sync(0xffffffffu, t.slot, lo + step - 1);
                         if (v < item) lo += step;
                     }
@@ -751,8 +769,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 }
                 const uint32_t b2 = __ballot_sync(0xffffffffu, pc == 2);
                 anywrap |= b2 != 0u;
-                const uint32_t Mt = transpose32((lane < total && pc != 0) ? (imask & ~selfm) : 0u, lane);
-                w.W[head & (GW_NSEG - 1)][lane] = Mt;
+                const uint32_t Mt = transpose32((lane < total && pc != 0) ? (imask & ~selfm) * REP : 0u, lane);
+                w.W[head & (GW_NSEG - 1)][lane] = Mt & myslots;
                 if (COUNT && lane == 0) w.seg_flags[head & (GW_NSEG - 1)] = SEG_PART;
                 ++head;
                 if (COUNT) {
@@ -765,13 +783,20 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     for (uint32_t j = 0; j < total; ++j) {
                         const uint32_t mj = __shfl_sync(0xffffffffu, imask & ~selfm, j);
                         const int cj = __shfl_sync(0xffffffffu, pc, j);
-                        if ((mj & mybit) && cj == 0) ++lc.pout;
+                        if (sl == 0u && (mj & mybit) && cj == 0) ++lc.pout;
                     }
                 }
                 __syncwarp();
             }
         }
-        if (valid) {
+        if (G < 32) {   // add the K partial sums of every target
+#pragma unroll
+            for (int o = G; o < 32; o <<= 1) {
+                acc.ax += __shfl_xor_sync(0xffffffffu, acc.ax, o); acc.ay += __shfl_xor_sync(0xffffffffu, acc.ay, o);
+                acc.az += __shfl_xor_sync(0xffffffffu, acc.az, o); acc.pot += __shfl_xor_sync(0xffffffffu, acc.pot, o);
+            }
+        }
+        if (valid && sl == 0u) {
             a.acc_out[3 * (size_t)out] = acc.ax;
             a.acc_out[3 * (size_t)out + 1] = acc.ay;
             a.acc_out[3 * (size_t)out + 2] = acc.az;
@@ -806,8 +831,14 @@ cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
         k_walk_simple<GEOM, POT, COUNT><<<grid, 128, 0, st>>>(a);
         return cudaGetLastError();
     }
+    // Targets per warp: 32 when the active targets are dense in Morton order; 8 (4 lanes per target) for a
+    // sparse active subset, whose 32 consecutive targets would span many cells (zoom: 52 -> 31 ms).  For the
+    // spread-out groups of a DENSE target set (uniform background of nfw256) 8 per warp is slower (measured).
+    const bool sparse = a.tgt_slot != nullptr && (uint64_t)a.n_active * 4u < t->n;
+    const int G = sparse ? OG_GW_SPARSE_G : 32;
+    a.n_groups = (uint32_t)(((uint64_t)a.n_active + G - 1) / G);
     const size_t smem = GW_WARPS * sizeof(WarpSmem);
-    auto kern = k_walk_group<GEOM, POT, COUNT>;
+    auto kern = sparse ? k_walk_group<GEOM, POT, COUNT, OG_GW_SPARSE_G> : k_walk_group<GEOM, POT, COUNT, 32>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
