@@ -361,7 +361,7 @@ struct LanePos {
 // iteration (two independent dependency chains).  Newtonian monopole x split factor in the loop (R21);
 // a source that is within OG_BAND of r_cut or closer than the largest softening length of the whole
 // particle set goes to pair_exact.  Returns the number of segments all lanes have finished.
-template <bool POT, bool COUNT, bool WRAP>
+template <bool POT, bool COUNT, bool WRAP, bool HLOOK>
 __device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, const uint32_t target, LanePos &lp,
                                             const Target &t, const float hmax2g, const WalkConst &c, Accum &acc,
                                             const uint32_t lane, unsigned long long *cnt, LaneCount &lc)
@@ -392,9 +392,26 @@ __device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, co
         }
         const float r20 = fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0));
         const float r21 = fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1));
-        // fast: strictly inside the cutoff band and beyond every softening length
-        const bool fast0 = v0 && r20 < c.rcut2_lo && r20 >= hmax2g;
-        const bool fast1 = v1 && r21 < c.rcut2_lo && r21 >= hmax2g;
+        // fast: strictly inside the cutoff band and not softened: anything closer than the largest h of the
+        // whole particle set (h_max of the root) takes the exact path.  HLOOK (the 8-targets-per-warp kernel,
+        // used for sparse active subsets, where a multi-species zoom has h comparable to r_cut): the source's
+        // own h is looked up below that bound (nodes carry h = 0: R16 keeps accepted nodes outside the
+        // target's own h).
+        bool fast0, fast1;
+        if (HLOOK) {
+            bool soft0 = r20 < hmax2g, soft1 = r21 < hmax2g;
+            float hj0 = 0.0f, hj1 = 0.0f;
+            if (v0 && soft0) hj0 = w.ring_h[e0];
+            if (v1 && soft1) hj1 = w.ring_h[e1];
+            const float hh0 = fmaxf(t.h, hj0), hh1 = fmaxf(t.h, hj1);
+            soft0 = soft0 && r20 < hh0 * hh0 * (1.0f + OG_BAND);
+            soft1 = soft1 && r21 < hh1 * hh1 * (1.0f + OG_BAND);
+            fast0 = v0 && r20 < c.rcut2_lo && !soft0;
+            fast1 = v1 && r21 < c.rcut2_lo && !soft1;
+        } else {
+            fast0 = v0 && r20 < c.rcut2_lo && r20 >= hmax2g;
+            fast1 = v1 && r21 < c.rcut2_lo && r21 >= hmax2g;
+        }
         const bool slow0 = v0 && !fast0 && r20 < c.rcut2_hi;
         const bool slow1 = v1 && !fast1 && r21 < c.rcut2_hi;
         {
@@ -538,8 +555,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 // ring full: free at least half of it; finishing: drain it
                 __syncwarp();
                 const uint32_t target = fin ? head : tail + GW_NSEG / 2;
-                tail = anywrap ? consume<POT, COUNT, true>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc)
-                               : consume<POT, COUNT, false>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc);
+                tail = anywrap ? consume<POT, COUNT, true, (G < 32)>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc)
+                               : consume<POT, COUNT, false, (G < 32)>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc);
                 __syncwarp();
             }
             if (fin) break;
