@@ -139,6 +139,9 @@ k_walk_simple(const __grid_constant__ WalkArgs a)
 #ifndef OG_GW_SPARSE_G
 #define OG_GW_SPARSE_G 8   // targets per warp for sparse active subsets (4, 8 or 16; zoom: 31.9 / 31.3 / 36.7 ms)
 #endif
+#ifndef OG_SPARSE_DIV
+#define OG_SPARSE_DIV 16u  // an active subset of fewer than n / 16 targets counts as sparse (10 % active: 77 ms at 32 per warp, 101 ms at 8)
+#endif
 #ifndef OG_GW_STACK
 #define OG_GW_STACK 256
 #endif
@@ -851,7 +854,7 @@ cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
     // Targets per warp: 32 when the active targets are dense in Morton order; 8 (4 lanes per target) for a
     // sparse active subset, whose 32 consecutive targets would span many cells (zoom: 52 -> 31 ms).  For the
     // spread-out groups of a DENSE target set (uniform background of nfw256) 8 per warp is slower (measured).
-    const bool sparse = a.tgt_slot != nullptr && (uint64_t)a.n_active * 4u < t->n;
+    const bool sparse = a.tgt_slot != nullptr && (uint64_t)a.n_active * OG_SPARSE_DIV < t->n;
     const int G = sparse ? OG_GW_SPARSE_G : 32;
     a.n_groups = (uint32_t)(((uint64_t)a.n_active + G - 1) / G);
     const size_t smem = GW_WARPS * sizeof(WarpSmem);
