@@ -173,3 +173,48 @@ def test_workspace_validate_and_host_entry(B):
     t3 = B.og_tree_build(badpos, mass, eps, w.L, prm)
     assert B.og_tree_status(t3) == B.OG_ERR_BAD_POSITION
     B.og_tree_free(t3)
+
+
+@pytest.mark.parametrize("G,rcut_over_rs,theta,alpha", [(2.5, 4.5, 0.5, 0.005), (1.0, 4.0, 0.7, 0.02), (0.3, 5.0, 0.3, 0.001)])
+def test_parameter_plumbing(B, G, rcut_over_rs, theta, alpha):
+    """G, rcut_over_rs (up to the polynomial's limit 5), theta and alpha other than the configs' values."""
+    w0 = W.make("nfw256", small=True)
+    w = W.Workload("params", w0.pos, w0.mass, w0.eps, w0.L, w0.r_s, alpha=alpha, theta=theta,
+                   rcut_over_rs=rcut_over_rs, G=G)
+    a1, p1, ao1, po1 = _both(B, w)
+    check_acc(a1, ao1, what="params geometric")
+    a_old = np.linalg.norm(ao1, axis=1).astype(np.float32)
+    a2, p2, ao2, po2 = _both(B, w, a_old=a_old)
+    check_acc(a2, ao2, what="params relative")
+    ep = rel_err_scalar(p2, po2)
+    assert np.percentile(ep, 99) <= 1e-4 and ep.max() <= 1e-2
+
+
+def test_rcut_over_rs_above_polynomial_range_is_rejected(B):
+    import torch
+    w = W.make("uniform32", small=True)
+    prm = B.make_params(w.r_s, rcut_over_rs=5.5)
+    with pytest.raises(B.OgError):
+        B.og_tree_build(*(torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps)), w.L, prm)
+    assert "rcut_over_rs" in B.og_last_error()
+
+
+def test_mixed_softening_species(B):
+    """Two species with very different softening (h of the heavy one comparable to r_cut), all active and a
+    sparse subset: spline branches, R16 guard with mixed h_max, both walk instantiations."""
+    rng = np.random.default_rng(21)
+    n_hi, n_lo = 30000, 6000
+    pos = np.concatenate([np.mod(0.5 + 0.05 * rng.standard_normal((n_hi, 3)), 1.0), rng.random((n_lo, 3))])
+    mass = np.concatenate([np.full(n_hi, 1.0), np.full(n_lo, 8.0)]) / (n_hi + 8.0 * n_lo)
+    eps = np.concatenate([np.full(n_hi, 0.001), np.full(n_lo, 0.012)])
+    w = _wl(pos, mass, eps)                      # r_cut = 0.0879, h_lo = 0.0336
+    a1, p1, ao1, po1 = _both(B, w)
+    check_acc(a1, ao1, what="species geometric")
+    a_old = np.linalg.norm(ao1, axis=1).astype(np.float32)
+    a2, p2, ao2, po2 = _both(B, w, a_old=a_old)
+    check_acc(a2, ao2, what="species relative")
+    act = np.sort(rng.choice(n_hi, 1500, replace=False)).astype(np.uint32)     # < n / 16: 8 targets per warp
+    a3, p3, ao3, po3 = _both(B, w, active=act, a_old=a_old[act])
+    check_acc(a3, ao3, what="species sparse")
+    ep = rel_err_scalar(p3, po3)
+    assert np.percentile(ep, 99) <= 1e-4 and ep.max() <= 1e-2
