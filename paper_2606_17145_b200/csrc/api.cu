@@ -167,8 +167,10 @@ extern "C" size_t og_tree_workspace_bytes(uint64_t n, const og_params *params)
     return make_layout(n, default_max_nodes(n, params), sms).total;
 }
 
-extern "C" og_tree *og_tree_build(const float *pos, const float *mass, const float *soft, uint64_t n,
-                                  float box, const og_params *params, og_stream stream)
+// og_tree_build; `before_gather` (may be NULL) is awaited on the stream before mass / soft are first read
+// (the HOST entry point copies them on a second stream while the keys are generated and sorted).
+static og_tree *tree_build_impl(const float *pos, const float *mass, const float *soft, uint64_t n,
+                                float box, const og_params *params, og_stream stream, cudaEvent_t before_gather)
 {
     g_err[0] = 0;
     if (!check_params(params, n, box)) return nullptr;
@@ -230,10 +232,17 @@ extern "C" og_tree *og_tree_build(const float *pos, const float *mass, const flo
     OG_BUILD_TRY(ogk_radix_sort(keysA, idxA, keysB, idxB, n, 0, 64, b + L.sort_scratch, &in_alt, st));
     t->keys = in_alt ? keysB : keysA;
     t->perm = in_alt ? idxB : idxA;
+    if (before_gather) OG_BUILD_TRY(cudaStreamWaitEvent(st, before_gather, 0));
     OG_BUILD_TRY(ogk_gather(pos, mass, soft, t->perm, n, t->spos, t->sh, t->inv_perm, st));
     OG_BUILD_TRY(ogk_octree_upward(t, b + L.oct_scratch, st));
 #undef OG_BUILD_TRY
     return t;
+}
+
+extern "C" og_tree *og_tree_build(const float *pos, const float *mass, const float *soft, uint64_t n,
+                                  float box, const og_params *params, og_stream stream)
+{
+    return tree_build_impl(pos, mass, soft, n, box, params, stream, nullptr);
 }
 
 extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx, uint64_t n_active,
@@ -408,18 +417,31 @@ extern "C" int og_shortrange_accel_host(const float *pos, const float *mass, con
     }
     int rc = OG_OK;
     og_tree *t = nullptr;
+    // Host-to-device copies run on a second stream so that they overlap the build: the keys and the sort
+    // need only pos, the gather waits for mass / soft, the walk for active_idx / a_old.
+    cudaStream_t cs = nullptr;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // buffer allocated, pos, mass + soft, the rest
 #define OG_H_TRY(expr) OG_CUDA_TRY(expr, { rc = OG_ERR_CUDA; goto done; })
-    OG_H_TRY(cudaMemcpyAsync(d + o_pos, pos, n * 12, cudaMemcpyHostToDevice, st));
-    OG_H_TRY(cudaMemcpyAsync(d + o_m, mass, n * 4, cudaMemcpyHostToDevice, st));
-    OG_H_TRY(cudaMemcpyAsync(d + o_s, soft, n * 4, cudaMemcpyHostToDevice, st));
-    if (active_idx) OG_H_TRY(cudaMemcpyAsync(d + o_ai, active_idx, na * 4, cudaMemcpyHostToDevice, st));
-    if (a_old) OG_H_TRY(cudaMemcpyAsync(d + o_ao, a_old, na * 4, cudaMemcpyHostToDevice, st));
+    OG_H_TRY(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+    for (int i = 0; i < 4; ++i) OG_H_TRY(cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming));
+    OG_H_TRY(cudaEventRecord(ev[0], st));
+    OG_H_TRY(cudaStreamWaitEvent(cs, ev[0], 0));
+    OG_H_TRY(cudaMemcpyAsync(d + o_pos, pos, n * 12, cudaMemcpyHostToDevice, cs));
+    OG_H_TRY(cudaEventRecord(ev[1], cs));
+    OG_H_TRY(cudaMemcpyAsync(d + o_m, mass, n * 4, cudaMemcpyHostToDevice, cs));
+    OG_H_TRY(cudaMemcpyAsync(d + o_s, soft, n * 4, cudaMemcpyHostToDevice, cs));
+    OG_H_TRY(cudaEventRecord(ev[2], cs));
+    if (active_idx) OG_H_TRY(cudaMemcpyAsync(d + o_ai, active_idx, na * 4, cudaMemcpyHostToDevice, cs));
+    if (a_old) OG_H_TRY(cudaMemcpyAsync(d + o_ao, a_old, na * 4, cudaMemcpyHostToDevice, cs));
+    OG_H_TRY(cudaEventRecord(ev[3], cs));
+    OG_H_TRY(cudaStreamWaitEvent(st, ev[1], 0));
     {
         og_params p = *params;
         p.workspace = nullptr; p.workspace_bytes = 0;
-        t = og_tree_build((const float *)(d + o_pos), (const float *)(d + o_m), (const float *)(d + o_s), n, box,
-                          &p, stream);
+        t = tree_build_impl((const float *)(d + o_pos), (const float *)(d + o_m), (const float *)(d + o_s), n, box,
+                            &p, stream, ev[2]);
     }
+    if (t) OG_H_TRY(cudaStreamWaitEvent(st, ev[3], 0));
     if (!t) { rc = OG_ERR_CUDA; goto done; }
     rc = og_shortrange_accel(t, active_idx ? (const uint32_t *)(d + o_ai) : nullptr, n_active,
                              a_old ? (const float *)(d + o_ao) : nullptr, (float *)(d + o_acc),
@@ -433,9 +455,12 @@ extern "C" int og_shortrange_accel_host(const float *pos, const float *mass, con
     }
 #undef OG_H_TRY
 done:
+    if (cs) cudaStreamSynchronize(cs);   // (on the error paths copies may still be in flight)
     if (t) og_tree_free(t, stream);
     cudaFreeAsync(d, st);
     cudaStreamSynchronize(st);
+    for (int i = 0; i < 4; ++i) if (ev[i]) cudaEventDestroy(ev[i]);
+    if (cs) cudaStreamDestroy(cs);
     return rc;
 }
 
