@@ -26,7 +26,7 @@ inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct Layout {
     size_t keysA, keysB, idxA, idxB, sort_scratch, spos, sh, inv_perm;
-    size_t level, first, count, first_child, nchild, com, cell, lo, hi, info, n1, n2;
+    size_t level, first, count, first_child, nchild, com, cell, lo, hi, info, rec;
     size_t oct_scratch, level_start, status, counters, small_end, spill, total;
 };
 
@@ -44,7 +44,7 @@ Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count)
     L.nchild = take(M);
     L.com = take(M * 16); L.cell = take(M * 16); L.lo = take(M * 16); L.hi = take(M * 16);
     L.info = take(M * 8);
-    L.n1 = take(M * 16); L.n2 = take(M * 16);
+    L.rec = take(M * 48);
     L.oct_scratch = take(ogk_octree_scratch_bytes(max_nodes));
     L.level_start = take(24 * 4);
     L.status = take(16 * 4);
@@ -214,7 +214,7 @@ static og_tree *tree_build_impl(const float *pos, const float *mass, const float
     t->node_nchild = (uint8_t *)(b + L.nchild);
     t->node_com = (float4 *)(b + L.com); t->node_cell = (float4 *)(b + L.cell);
     t->node_lo = (float4 *)(b + L.lo); t->node_hi = (float4 *)(b + L.hi); t->node_info = (uint2 *)(b + L.info);
-    t->node_n1 = (uint4 *)(b + L.n1); t->node_n2 = (float4 *)(b + L.n2);
+    t->node_rec = (uint4 *)(b + L.rec);
     t->d_level_start = (uint32_t *)(b + L.level_start); t->d_status = (uint32_t *)(b + L.status);
     t->d_counters = (unsigned long long *)(b + L.counters);
     t->walk_spill = b + L.spill; t->walk_spill_bytes = ogk_walk_spill_bytes(sms);

@@ -211,8 +211,7 @@ struct UpArgs {
     double4 *sums;      // (M, sum m x, sum m y, sum m z) per node, fp64
     float4 *com, *cell, *lo, *hi;
     uint2 *info;
-    uint4 *n1;
-    float4 *n2;
+    uint4 *rec;         // packed walk records, 3 x 16 B per node
     uint32_t *status;
 };
 
@@ -326,8 +325,10 @@ k_upward(UpArgs a)
         const uint32_t cnt = info.y & ~OG_LEAF_BIT;
         if (cnt >= (1u << 26)) atomicOr(a.status, OG_DEV_NODE_OVERFLOW);   // does not fit the packed record
         const uint32_t meta = ((uint32_t)a.level[j] << 27) | (leaf << 26) | (cnt & 0x03ffffffu);
-        a.n1[j] = make_uint4(__float_as_uint(R), __float_as_uint(fmaxf(rg, lo.w)), info.x, meta);
-        a.n2[j] = make_float4(cc.x, cc.y, cc.z, lo.w);
+        uint4 *r = a.rec + 3 * (size_t)j;
+        r[0] = make_uint4(__float_as_uint(s.x), __float_as_uint(s.y), __float_as_uint(s.z), __float_as_uint(s.w));
+        r[1] = make_uint4(__float_as_uint(R), __float_as_uint(fmaxf(rg, lo.w)), info.x, meta);
+        r[2] = make_uint4(__float_as_uint(cc.x), __float_as_uint(cc.y), __float_as_uint(cc.z), __float_as_uint(lo.w));
     }
 }
 
@@ -364,7 +365,7 @@ cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st)
     if (e != cudaSuccess) return e;
     UpArgs ua{t->keys, t->spos, t->sh, t->box, t->node_level, t->node_first, t->node_count,
               t->node_first_child, t->node_nchild, t->d_level_start, sums, t->node_com, t->node_cell,
-              t->node_lo, t->node_hi, t->node_info, t->node_n1, t->node_n2, t->d_status};
+              t->node_lo, t->node_hi, t->node_info, t->node_rec, t->d_status};
     void *args2[] = {&ua};
     e = cudaLaunchCooperativeKernel((const void *)k_upward,
                                     dim3(coop_grid((const void *)k_upward, OCT_THREADS, t->sm_count)),

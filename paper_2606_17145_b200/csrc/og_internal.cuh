@@ -60,13 +60,12 @@ struct og_tree {
     float4 *node_hi;
     uint2 *node_info;
     // packed walk records (read by the group walk; written by the last phase of k_upward):
-    //   n0 = node_com
+    //   n0 = node_com (copied, so that the three quadwords of a node are contiguous)
     //   n1 = (R, ng, first, meta): R = largest distance from s to a corner of the AABB (rounded up),
     //        ng = max(h_max, largest |x - s| over the 0.6 l guard box of R15) (rounded up), first = first
     //        child / first slot, meta = level << 27 | leaf << 26 | (n_child or particle count)
     //   n2 = (c_x, c_y, c_z, h_max)
-    uint4 *node_n1;
-    float4 *node_n2;
+    uint4 *node_rec;           // [3 n_nodes]: n0, n1, n2 of node j at 3 j, 3 j + 1, 3 j + 2 (48 contiguous bytes)
     // small device state
     uint32_t *d_level_start;   // [24]: start index per level, [22] = n_nodes, [23] = max level
     uint32_t *d_status;        // [4]: latched status bits, walk work counter, ...

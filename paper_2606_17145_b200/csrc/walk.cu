@@ -29,8 +29,7 @@ namespace {
 struct WalkArgs {
     const float4 *com, *cell, *lo, *hi;   // full node records (exact path, simple walk); com doubles as n0
     const uint2 *info;
-    const uint4 *n1;           // packed walk record (R, ng, first, meta), og_internal.cuh
-    const float4 *n2;          // (c_x, c_y, c_z, h_max)
+    const uint4 *rec;          // packed walk records (n0, n1, n2), 48 contiguous bytes per node, og_internal.cuh
     const float4 *spos;
     const float *sh;
     const uint32_t *tgt_slot;  // NULL -> identity
@@ -571,9 +570,10 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 int cls = CL_DROP;
                 bool shifted = true;
                 if (lane < total) {
-                    const float4 n0 = __ldg(a.com + item);
-                    const uint4 n1 = __ldg(a.n1 + item);
-                    const float4 n2 = __ldg(a.n2 + item);
+                    const uint4 *rp = a.rec + 3 * (size_t)item;
+                    const uint4 r0 = __ldg(rp), n1 = __ldg(rp + 1), r2 = __ldg(rp + 2);
+                    const float4 n0 = make_float4(__uint_as_float(r0.x), __uint_as_float(r0.y), __uint_as_float(r0.z), __uint_as_float(r0.w));
+                    const float4 n2 = make_float4(__uint_as_float(r2.x), __uint_as_float(r2.y), __uint_as_float(r2.z), __uint_as_float(r2.w));
                     first = n1.z; meta = n1.w;
                     const float l = c.L * __uint_as_float((127u - (meta >> 27)) << 23);   // L / 2^level, exact
                     float4 sc, aux;
@@ -885,7 +885,7 @@ cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t 
 {
     WalkArgs a;
     a.com = t->node_com; a.cell = t->node_cell; a.lo = t->node_lo; a.hi = t->node_hi;
-    a.info = t->node_info; a.n1 = t->node_n1; a.n2 = t->node_n2; a.spos = t->spos; a.sh = t->sh;
+    a.info = t->node_info; a.rec = t->node_rec; a.spos = t->spos; a.sh = t->sh;
     a.tgt_slot = tgt_slot; a.tgt_out = tgt_out; a.a_old = a_old; a.acc_out = acc_out; a.pot_out = pot_out;
     a.n_active = (uint32_t)n_active;
     a.n_groups = (uint32_t)((n_active + 31) / 32);
