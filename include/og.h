@@ -61,7 +61,8 @@ typedef struct {
     uint32_t flags;         /* OG_PERIODIC | ...                                           */
     float G;                /* gravitational constant (R12; 1 in all configs)              */
     float r_s;              /* force-split scale, same units as box                        */
-    float rcut_over_rs;     /* 4.5 (BASELINE.json north_star)                              */
+    float rcut_over_rs;     /* 4.5 (BASELINE.json north_star); must be <= 5 (range of the  */
+                            /* split-factor polynomial)                */
     float alpha;            /* relative opening criterion (R14), used iff a_old != NULL    */
     float theta;            /* geometric criterion (R22), used iff a_old == NULL           */
     uint32_t leaf_max;      /* bucket size of the canonical octree (R7), default 8         */
@@ -141,7 +142,10 @@ og_tree *og_tree_build(const float *pos, const float *mass, const float *soft, u
  *              NULL -> geometric criterion l^2 > theta^2 r^2 (R22)
  *   acc_out    DEVICE f32 [n_active][3], overwritten (n_active == 0: nothing is done, OG_OK)
  *   pot_out    DEVICE f32 [n_active], overwritten, or NULL
- * Returns OG_OK or a negative og_status (also a previously latched device condition).
+ * Returns OG_OK or a negative og_status; conditions detected on the device (bad index, traversal stack
+ * capacity) are latched and reported by og_tree_status().  n_active == 0 is a no-op.  Implementation note:
+ * 32 targets per warp; an active subset of fewer than n / 16 targets is walked with 8 targets per warp
+ * (4 lanes per target).  Results do not depend on the launch order (bit-reproducible run to run).
  */
 int og_shortrange_accel(const og_tree *tree, const uint32_t *active_idx, uint64_t n_active,
                         const float *a_old, float *acc_out, float *pot_out, og_stream stream);
