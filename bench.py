@@ -65,6 +65,25 @@ def ncu_traffic(name):
     return None
 
 
+def fp32_probe(iters=100000):
+    """Measured FP32 rates (TFLOP/s) of the scalar FFMA and the packed FFMA2 encoding, from the bench-side helper
+    library libogprobe.so (csrc/probe.cu; not part of libogtree.so).  None if the helper is missing."""
+    import ctypes as C
+    path = os.path.join(ROOT, "paper_2606_17145_b200", "libogprobe.so")
+    if not os.path.exists(path):
+        return None
+    lib = C.CDLL(path)
+    lib.ogp_fp32_probe.restype = C.c_int
+    lib.ogp_fp32_probe.argtypes = [C.c_int, C.c_uint64, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    out = {}
+    for mode, name in ((0, "ffma"), (1, "ffma2")):
+        ms, fl = C.c_double(), C.c_double()
+        if lib.ogp_fp32_probe(mode, iters, C.byref(ms), C.byref(fl)) != 0 or ms.value <= 0:
+            return None
+        out[name] = fl.value / (ms.value * 1e-3) / 1e12
+    return out
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -239,6 +258,8 @@ def run_reference(args):
             "config": {"workload": args.workload, "n": w.n, "n_active": w.n_active},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                              "sample": sample},
+            # ms_per_step is not a measured wall time: walk of `sample_targets` targets scaled to all active ones
+            "extrapolated": True, "sample_targets": int(ns), "tree_build_s": t_build, "walk_sample_s": t_walk,
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -356,21 +377,25 @@ def run_ours(args):
         inter = units["interactions_per_target"] * na
         units_src = "oracle-counted per-target figure (algorithmic_units.json) x active targets"
     else:
-        F_alg, F_int, inter = float(F_gpu), None, float(stc["A_in"] + stc["P_in"])
-        units_src = "GPU OG_COUNT counters (no oracle figure for this workload)"
-    achieved = F_alg / (ms_walk * 1e-3) / 1e12
-    ffma_ms, ffma_fl = B.og_ffma_peak_probe(100000)
+        # no oracle-counted figure for this workload: no algorithmic flops, hence no roofline fraction (the
+        # kernel's own OG_COUNT counters are reported beside it but never grade the kernel)
+        F_alg, F_int, inter = None, None, float(stc["A_in"] + stc["P_in"])
+        units_src = "none: no oracle-counted figure in algorithmic_units.json for this workload (run oracle/count_units.py)"
+    achieved = F_alg / (ms_walk * 1e-3) / 1e12 if F_alg else None
+    probe = fp32_probe()
     t_hbm_ms = (units["compulsory_hbm_bytes"] if units else 0) / (float(peaks["hbm_gbs"]) * 1e9) * 1e3
     roofline = {
         "bound": "alu", "kernel": "k_walk_group", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved / peak_tflops, "traffic": ncu_traffic(w.name),
+        "frac": achieved / peak_tflops if achieved else None, "traffic": ncu_traffic(w.name),
+        "traffic_source": f"profiles/walk_traffic_{w.name}.txt (one committed ncu --set full capture; not measured in this run)",
         "peak_source": f"{sms} SMs x {SM_LANES} FP32 lanes x 2 flop x {fmax / 1e6:.0f} MHz (max SM clock, "
                        f"MEASURED_PEAKS.json {peaks_src}); DESIGN.md Sec. 7",
         "algorithmic_flops_per_launch": F_alg, "units": units_src,
         "frac_interactions_only": (F_int / (ms_walk * 1e-3) / 1e12 / peak_tflops) if F_int else None,
         "algorithmic_flops_gpu_counters": float(F_gpu),
-        "ffma_probe_tflops": ffma_fl / (ffma_ms * 1e-3) / 1e12,
-        "hbm_bound_ms": t_hbm_ms, "alu_bound_ms": F_alg / (peak_tflops * 1e12) * 1e3,
+        "ffma_probe_tflops": probe["ffma"] if probe else None,
+        "ffma2_probe_tflops": probe["ffma2"] if probe else None,
+        "hbm_bound_ms": t_hbm_ms, "alu_bound_ms": F_alg / (peak_tflops * 1e12) * 1e3 if F_alg else None,
         "kernel_ms": ms_walk, "kernel_share_of_step": ms_walk / (ms_build + ms_walk),
     }
     line = {

@@ -15,6 +15,13 @@
  *  - `stream` is a cudaStream_t passed as an opaque pointer (NULL = legacy default
  *    stream).  Calls only ENQUEUE work on `stream` and return; the library never calls
  *    cudaDeviceSynchronize.  Inputs must stay valid until the stream has passed the call.
+ *  - Streams and a tree: og_shortrange_accel may be called on any stream.  The library orders it
+ *    after the tree's build and after the previous walk on the same tree (events; no host
+ *    synchronisation), because a walk uses scratch state owned by the tree (group counter,
+ *    traversal-stack slabs, OG_COUNT counters): walks on ONE tree therefore run one after the
+ *    other even when issued on different streams; walks on different trees overlap freely.
+ *    og_tree_free orders the release after the last walk.  Calls on one tree from several host
+ *    threads at the same time are not supported.
  *  - `int` functions return OG_OK (0) or a negative og_status; og_tree_build returns NULL
  *    on synchronous failure.  og_last_error() holds a thread-local message for the last
  *    failing call.  No C++ exception crosses the ABI; nothing aborts.
@@ -52,10 +59,6 @@ typedef enum {
 #define OG_VALIDATE_POS 2u  /* device-side check 0 <= x < box during key generation       */
 #define OG_COUNT 4u         /* walk also accumulates interaction counters (og_stats)      */
 
-/* og_params.walk_variant */
-#define OG_WALK_DEFAULT 0u  /* warp-cooperative group walk (the product path)             */
-#define OG_WALK_SIMPLE 1u   /* one thread per target, private stack (debug / comparison)  */
-
 typedef struct {
     uint32_t struct_size;   /* = sizeof(og_params); ABI guard                              */
     uint32_t flags;         /* OG_PERIODIC | ...                                           */
@@ -67,7 +70,11 @@ typedef struct {
     float theta;            /* geometric criterion (R22), used iff a_old == NULL           */
     uint32_t leaf_max;      /* bucket size of the canonical octree (R7), default 8         */
     uint32_t max_nodes;     /* node capacity; 0 -> default (R6)                            */
-    uint32_t walk_variant;  /* OG_WALK_*                                                   */
+    /* additions over SURVEY.md Sec. 8.2 (capacity knobs of the walk's traversal stack; 0 -> default): */
+    uint32_t walk_stack_entries;  /* pending node ranges a warp keeps in shared memory before it spills the
+                                     older half to its global slab (default and maximum 256)               */
+    uint32_t walk_spill_entries;  /* capacity of that global slab per warp, in ranges (default 3072);
+                                     exceeding it latches OG_ERR_STACK_OVERFLOW                            */
     void *workspace;        /* DEVICE scratch supplied by the caller, or NULL -> the       */
     size_t workspace_bytes; /* library allocates with cudaMallocAsync on `stream`          */
 } og_params;
@@ -89,7 +96,7 @@ typedef struct {
      * all / accepted by all / undecided; particles dropped / staged shifted / staged for per-lane
      * wrap; node batches popped                                                              */
     uint64_t cl_drop, cl_open, cl_accept, cl_generic, pt_drop, pt_shift, pt_wrap, batches;
-    uint64_t diag[32];      /* implementation diagnostics of the walk kernel (OG_COUNT); meaning may change */
+    uint64_t stack_spills;  /* times a warp moved half of its traversal stack to its global slab        */
 } og_stats;
 
 /* og_tree_get field selectors.  Pointers are DEVICE pointers into the tree, valid until
@@ -195,10 +202,11 @@ int og_shortrange_accel_host(const float *pos, const float *mass, const float *s
                              uint64_t n_active, const float *a_old, float *acc_out,
                              float *pot_out, og_stream stream);
 
-/* FP32 FFMA micro-benchmark used by bench.py to state the measured ALU peak next to the
- * nominal one: runs `iters` dependent-chain FFMAs x 8 chains per thread on every SM and
- * returns the elapsed milliseconds (CUDA events, synchronises) and the flop count.        */
-int og_ffma_peak_probe(uint64_t iters, double *ms_out, double *flops_out, og_stream stream);
+/* Returns the device memory that freed trees / finished calls left cached in the library's
+ * stream-ordered pool of the current device to the driver (the pool keeps arenas for reuse by
+ * the next og_tree_build; a host code that needs the memory for something else calls this).
+ * Synchronises nothing; memory still in use stays.                                         */
+int og_trim(void);
 
 #ifdef __cplusplus
 }

@@ -27,9 +27,6 @@ OG_ERR_STACK_OVERFLOW = -6
 OG_PERIODIC = 1
 OG_VALIDATE_POS = 2
 OG_COUNT = 4
-# walk variants
-OG_WALK_DEFAULT = 0
-OG_WALK_SIMPLE = 1
 # og_field
 (OG_F_KEYS_SORTED, OG_F_PERM, OG_F_INV_PERM, OG_F_SPOS, OG_F_SH, OG_F_NODE_LEVEL, OG_F_NODE_FIRST,
  OG_F_NODE_COUNT, OG_F_NODE_FIRST_CHILD, OG_F_NODE_NCHILD, OG_F_NODE_COM, OG_F_NODE_CELL, OG_F_NODE_LO,
@@ -52,8 +49,8 @@ class OgError(RuntimeError):
 class og_params(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("flags", C.c_uint32), ("G", C.c_float), ("r_s", C.c_float),
                 ("rcut_over_rs", C.c_float), ("alpha", C.c_float), ("theta", C.c_float),
-                ("leaf_max", C.c_uint32), ("max_nodes", C.c_uint32), ("walk_variant", C.c_uint32),
-                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+                ("leaf_max", C.c_uint32), ("max_nodes", C.c_uint32), ("walk_stack_entries", C.c_uint32),
+                ("walk_spill_entries", C.c_uint32), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
 
 
 class og_stats(C.Structure):
@@ -62,18 +59,16 @@ class og_stats(C.Structure):
                 ("P_soft", C.c_uint64), ("P_out", C.c_uint64), ("fp64_rechecks", C.c_uint64),
                 ("cl_drop", C.c_uint64), ("cl_open", C.c_uint64), ("cl_accept", C.c_uint64),
                 ("cl_generic", C.c_uint64), ("pt_drop", C.c_uint64), ("pt_shift", C.c_uint64),
-                ("pt_wrap", C.c_uint64), ("batches", C.c_uint64), ("diag", C.c_uint64 * 32)]
+                ("pt_wrap", C.c_uint64), ("batches", C.c_uint64), ("stack_spills", C.c_uint64)]
 
     def as_dict(self):
-        d = {k: int(getattr(self, k)) for k, _ in self._fields_ if k not in ("reserved", "diag")}
-        d["diag"] = [int(x) for x in self.diag]
-        return d
+        return {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}
 
 
 def make_params(r_s, G=1.0, rcut_over_rs=4.5, alpha=0.005, theta=0.5, leaf_max=8, max_nodes=0, flags=OG_PERIODIC,
-                walk_variant=OG_WALK_DEFAULT) -> og_params:
+                walk_stack_entries=0, walk_spill_entries=0) -> og_params:
     return og_params(C.sizeof(og_params), flags | OG_PERIODIC, G, r_s, rcut_over_rs, alpha, theta, leaf_max,
-                     max_nodes, walk_variant, None, 0)
+                     max_nodes, walk_stack_entries, walk_spill_entries, None, 0)
 
 
 def _load():
@@ -108,8 +103,8 @@ def _load():
     lib.og_shortrange_accel_host.restype = C.c_int
     lib.og_shortrange_accel_host.argtypes = [vp, vp, vp, u64, C.c_float, C.POINTER(og_params), vp, u64, vp, vp,
                                              vp, vp]
-    lib.og_ffma_peak_probe.restype = C.c_int
-    lib.og_ffma_peak_probe.argtypes = [u64, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
+    lib.og_trim.restype = C.c_int
+    lib.og_trim.argtypes = []
     return lib
 
 
@@ -117,7 +112,7 @@ _lib = _load()
 
 EXPORTS = ("og_tree_workspace_bytes", "og_tree_build", "og_shortrange_accel", "og_tree_get", "og_tree_status",
            "og_tree_stats", "og_tree_free", "og_last_error", "og_morton_keys", "og_radix_sort_scratch_bytes",
-           "og_radix_sort_pairs", "og_shortrange_accel_host", "og_ffma_peak_probe")
+           "og_radix_sort_pairs", "og_shortrange_accel_host", "og_trim")
 
 
 def _err() -> str:
@@ -296,8 +291,6 @@ def og_shortrange_accel_host(pos, mass, soft, box: float, params: og_params, act
     return acc_out, pot_out
 
 
-def og_ffma_peak_probe(iters: int = 200000, stream=None):
-    """-> (milliseconds, flops) of the FFMA-only probe kernel."""
-    ms, fl = C.c_double(), C.c_double()
-    _check(_lib.og_ffma_peak_probe(iters, C.byref(ms), C.byref(fl), _stream(stream)))
-    return ms.value, fl.value
+def og_trim():
+    """Returns the memory cached in the library's stream-ordered pool to the driver."""
+    _check(_lib.og_trim())

@@ -1,4 +1,5 @@
-"""Builds libogtree.so (hand-written CUDA for sm_100a) in-tree with nvcc.
+"""Builds libogtree.so (hand-written CUDA for sm_100a; the product) and libogprobe.so (the FP32 throughput
+probe bench.py uses to state the measured ALU rate; not part of the product ABI) in-tree with nvcc.
 
     python -m paper_2606_17145_b200.build [--force]
 
@@ -15,7 +16,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libogtree.so")
-SOURCES = ["api.cu", "keys.cu", "radix_sort.cu", "octree.cu", "walk.cu", "probe.cu"]
+PROBE_LIB = os.path.join(HERE, "libogprobe.so")
+SOURCES = ["api.cu", "keys.cu", "radix_sort.cu", "octree.cu", "walk.cu"]
+PROBE_SOURCES = ["probe.cu"]
 HEADERS = ["og_internal.cuh", "walk_math.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
@@ -29,10 +32,10 @@ def _nvcc() -> str:
 
 
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(PROBE_LIB):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.join(ROOT, "include", "og.h"),
+    t = min(os.path.getmtime(LIB), os.path.getmtime(PROBE_LIB))
+    deps = [os.path.join(CSRC, s) for s in SOURCES + PROBE_SOURCES + HEADERS] + [os.path.join(ROOT, "include", "og.h"),
                                                                   os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
@@ -44,7 +47,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(objdir, exist_ok=True)
     objs = []
     procs = []
-    for s in SOURCES:
+    for s in SOURCES + PROBE_SOURCES:
         o = os.path.join(objdir, s.replace(".cu", ".o"))
         cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("OG_NVCC_EXTRA", "").split(), "-I", os.path.join(ROOT, "include"), "-I", CSRC, "-c",
                os.path.join(CSRC, s), "-o", o]
@@ -62,7 +65,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         sys.stderr.write("\n".join(log))
     if failed:
         raise RuntimeError("nvcc failed (see output above)")
-    subprocess.run([_nvcc(), "-shared", "-o", LIB, *objs], check=True)  # static cudart (nvcc default)
+    n = len(SOURCES)
+    subprocess.run([_nvcc(), "-shared", "-o", LIB, *objs[:n]], check=True)  # static cudart (nvcc default)
+    subprocess.run([_nvcc(), "-shared", "-o", PROBE_LIB, *objs[n:]], check=True)
     return LIB
 
 

@@ -30,7 +30,7 @@ struct Layout {
     size_t oct_scratch, level_start, status, counters, small_end, spill, total;
 };
 
-Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count)
+Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count, uint32_t spill_entries)
 {
     Layout L;
     size_t o = 0;
@@ -50,7 +50,7 @@ Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count)
     L.status = take(16 * 4);
     L.counters = take(OGC_N * 8);
     L.small_end = o;
-    L.spill = take(ogk_walk_spill_bytes(sm_count));
+    L.spill = take(ogk_walk_spill_bytes(sm_count, spill_entries));
     L.total = o;
     return L;
 }
@@ -86,7 +86,11 @@ bool check_params(const og_params *p, uint64_t n, float box)
                      (double)p->rcut_over_rs * (double)p->r_s, 0.5 * (double)box);
         return false;
     }
-    if (p->walk_variant > OG_WALK_SIMPLE) { og_set_error("unknown walk_variant %u", p->walk_variant); return false; }
+    if (p->walk_stack_entries != 0 && (p->walk_stack_entries < 64 || p->walk_stack_entries > 256 || (p->walk_stack_entries & 1u))) {
+        og_set_error("walk_stack_entries = %u: must be 0 (default) or an even number in [64, 256]", p->walk_stack_entries);
+        return false;
+    }
+    if (p->walk_spill_entries > (1u << 20)) { og_set_error("walk_spill_entries = %u: at most 2^20", p->walk_spill_entries); return false; }
     return true;
 }
 
@@ -103,10 +107,13 @@ int device_sm_count(int *device_out)
 // unlimited: a tree arena (GBs) freed by og_tree_free is reused by the next og_tree_build instead
 // of going back to the driver at every synchronisation (the default pool's behaviour, ~16 ms per
 // 3 GB arena on B200).
+std::mutex g_pool_mu;
+cudaMemPool_t g_pools[64] = {};
+
 cudaError_t og_malloc_async(void **ptr, size_t bytes, cudaStream_t st)
 {
-    static std::mutex mu;
-    static cudaMemPool_t pools[64] = {};
+    std::mutex &mu = g_pool_mu;
+    cudaMemPool_t *pools = g_pools;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
@@ -142,8 +149,8 @@ int status_from_bits(uint32_t bits)
 // Synchronises the streams the tree has been used on and refreshes the host copies.
 int tree_sync(const og_tree *t, uint32_t *bits_out)
 {
-    OG_CUDA_TRY(cudaStreamSynchronize(t->build_stream), return OG_ERR_CUDA);
-    if (t->last_stream != t->build_stream) OG_CUDA_TRY(cudaStreamSynchronize(t->last_stream), return OG_ERR_CUDA);
+    OG_CUDA_TRY(cudaEventSynchronize(t->ev_built), return OG_ERR_CUDA);
+    if (t->walked) OG_CUDA_TRY(cudaEventSynchronize(t->ev_walked), return OG_ERR_CUDA);
     uint32_t ls[24];
     OG_CUDA_TRY(cudaMemcpy(ls, t->d_level_start, sizeof(ls), cudaMemcpyDeviceToHost), return OG_ERR_CUDA);
     t->n_nodes_host = ls[22];
@@ -157,6 +164,13 @@ int tree_sync(const og_tree *t, uint32_t *bits_out)
     return OG_OK;
 }
 
+void tree_delete(og_tree *t)
+{
+    if (t->ev_built) cudaEventDestroy(t->ev_built);
+    if (t->ev_walked) cudaEventDestroy(t->ev_walked);
+    delete t;
+}
+
 }  // namespace
 
 extern "C" size_t og_tree_workspace_bytes(uint64_t n, const og_params *params)
@@ -164,7 +178,7 @@ extern "C" size_t og_tree_workspace_bytes(uint64_t n, const og_params *params)
     if (!params || params->struct_size != sizeof(og_params) || n == 0 || n >= (1ull << 31)) return 0;
     int sms = device_sm_count(nullptr);
     if (sms <= 0) sms = 148;  // no device visible: size for a B200
-    return make_layout(n, default_max_nodes(n, params), sms).total;
+    return make_layout(n, default_max_nodes(n, params), sms, ogk_walk_spill_entries(params)).total;
 }
 
 // og_tree_build; `before_gather` (may be NULL) is awaited on the stream before mass / soft are first read
@@ -184,13 +198,22 @@ static og_tree *tree_build_impl(const float *pos, const float *mass, const float
     memset(t, 0, sizeof(*t));
     t->n = n; t->box = box; t->prm = *params; t->device = dev; t->sm_count = sms;
     t->max_nodes = default_max_nodes(n, params);
-    t->build_stream = st; t->last_stream = st; t->n_nodes_host = -1;
-    const Layout L = make_layout(n, t->max_nodes, sms);
+    t->build_stream = st; t->n_nodes_host = -1;
+    t->walk_spill_cap = ogk_walk_spill_entries(params);
+    if (cudaEventCreateWithFlags(&t->ev_built, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&t->ev_walked, cudaEventDisableTiming) != cudaSuccess) {
+        og_set_error("cudaEventCreate failed");
+        (void)cudaGetLastError();
+        if (t->ev_built) cudaEventDestroy(t->ev_built);
+        delete t;
+        return nullptr;
+    }
+    const Layout L = make_layout(n, t->max_nodes, sms, t->walk_spill_cap);
     if (params->workspace) {
         if (params->workspace_bytes < L.total || ((uintptr_t)params->workspace & 255u)) {
             og_set_error("workspace too small or not 256-byte aligned: %zu bytes given, %zu needed",
                          params->workspace_bytes, L.total);
-            delete t;
+            tree_delete(t);
             return nullptr;
         }
         t->arena = params->workspace; t->owns_arena = 0;
@@ -199,7 +222,7 @@ static og_tree *tree_build_impl(const float *pos, const float *mass, const float
         if (e != cudaSuccess) {
             og_set_error("cudaMallocAsync(%zu bytes) failed: %s", L.total, cudaGetErrorString(e));
             (void)cudaGetLastError();
-            delete t;
+            tree_delete(t);
             return nullptr;
         }
         t->owns_arena = 1;
@@ -217,12 +240,12 @@ static og_tree *tree_build_impl(const float *pos, const float *mass, const float
     t->node_rec = (uint4 *)(b + L.rec);
     t->d_level_start = (uint32_t *)(b + L.level_start); t->d_status = (uint32_t *)(b + L.status);
     t->d_counters = (unsigned long long *)(b + L.counters);
-    t->walk_spill = b + L.spill; t->walk_spill_bytes = ogk_walk_spill_bytes(sms);
+    t->walk_spill = b + L.spill; t->walk_spill_bytes = ogk_walk_spill_bytes(sms, t->walk_spill_cap);
 
 #define OG_BUILD_TRY(expr)                                                    \
     OG_CUDA_TRY(expr, {                                                       \
         if (t->owns_arena) cudaFreeAsync(t->arena, st);                       \
-        delete t;                                                             \
+        tree_delete(t);                                                       \
         return nullptr;                                                       \
     })
     // level_start, status, counters are adjacent: clear them in one memset
@@ -235,6 +258,7 @@ static og_tree *tree_build_impl(const float *pos, const float *mass, const float
     if (before_gather) OG_BUILD_TRY(cudaStreamWaitEvent(st, before_gather, 0));
     OG_BUILD_TRY(ogk_gather(pos, mass, soft, t->perm, n, t->spos, t->sh, t->inv_perm, st));
     OG_BUILD_TRY(ogk_octree_upward(t, b + L.oct_scratch, st));
+    OG_BUILD_TRY(cudaEventRecord(t->ev_built, st));
 #undef OG_BUILD_TRY
     return t;
 }
@@ -259,9 +283,13 @@ extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx,
     }
     if (n_active >= (1ull << 31)) { og_set_error("n_active out of range"); return OG_ERR_INVALID_ARG; }
     cudaStream_t st = (cudaStream_t)stream;
-    t->last_stream = st;
+    // after the build, and after the previous walk on this tree (its scratch state is shared): og.h
+    if (st != t->build_stream) OG_CUDA_TRY(cudaStreamWaitEvent(st, t->ev_built, 0), return OG_ERR_CUDA);
+    if (t->walked) OG_CUDA_TRY(cudaStreamWaitEvent(st, t->ev_walked, 0), return OG_ERR_CUDA);
     if (!active_idx) {
         OG_CUDA_TRY(ogk_walk(t, nullptr, t->perm, n_active, a_old, acc_out, pot_out, st), return OG_ERR_CUDA);
+        OG_CUDA_TRY(cudaEventRecord(t->ev_walked, st), return OG_ERR_CUDA);
+        t->walked = true;
         return OG_OK;
     }
     // active subset: order the targets by sorted slot so that a warp's 32 targets are neighbours
@@ -286,6 +314,8 @@ extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx,
     OG_ACC_TRY(ogk_radix_sort(k0, v0, k1, v1, n_active, 0, bits, tmp + o_sc, &in_alt, st));
     OG_ACC_TRY(ogk_unpack_slots(in_alt ? k1 : k0, n_active, slots, st));
     OG_ACC_TRY(ogk_walk(t, slots, in_alt ? v1 : v0, n_active, a_old, acc_out, pot_out, st));
+    OG_ACC_TRY(cudaEventRecord(t->ev_walked, st));
+    t->walked = true;
     OG_ACC_TRY(cudaFreeAsync(tmp, st));
 #undef OG_ACC_TRY
     return OG_OK;
@@ -349,7 +379,7 @@ extern "C" int og_tree_stats(const og_tree *t, og_stats *out)
     out->cl_drop = c[OGC_CL_DROP]; out->cl_open = c[OGC_CL_OPEN]; out->cl_accept = c[OGC_CL_ACCEPT];
     out->cl_generic = c[OGC_CL_GENERIC]; out->pt_drop = c[OGC_PT_DROP]; out->pt_shift = c[OGC_PT_SHIFT];
     out->pt_wrap = c[OGC_PT_WRAP]; out->batches = c[OGC_BATCHES];
-    for (int i = 0; i < 32; ++i) out->diag[i] = c[OGC_DIAG0 + i];
+    out->stack_spills = c[OGC_SPILLS];
     return OG_OK;
 }
 
@@ -357,11 +387,12 @@ extern "C" void og_tree_free(og_tree *t, og_stream stream)
 {
     if (!t) return;
     if (t->owns_arena && t->arena) {
-        // the arena may still be in use on another stream: order the free after it
-        if (t->last_stream != (cudaStream_t)stream) cudaStreamSynchronize(t->last_stream);
+        // the arena may still be in use by the build or the last walk on another stream: order the free after them
+        cudaStreamWaitEvent((cudaStream_t)stream, t->ev_built, 0);
+        if (t->walked) cudaStreamWaitEvent((cudaStream_t)stream, t->ev_walked, 0);
         cudaFreeAsync(t->arena, (cudaStream_t)stream);
     }
-    delete t;
+    tree_delete(t);
 }
 
 extern "C" int og_morton_keys(const float *pos, uint64_t n, float box, uint64_t *keys, uint32_t *idx,
@@ -464,30 +495,17 @@ done:
     return rc;
 }
 
-extern "C" int og_ffma_peak_probe(uint64_t iters, double *ms_out, double *flops_out, og_stream stream)
+extern "C" int og_trim(void)
 {
     g_err[0] = 0;
-    if (!ms_out || !flops_out || iters == 0) { og_set_error("bad argument"); return OG_ERR_INVALID_ARG; }
-    const int sms = device_sm_count(nullptr);
-    if (sms <= 0) { og_set_error("no CUDA device available"); return OG_ERR_CUDA; }
-    cudaStream_t st = (cudaStream_t)stream;
-    float *sink = nullptr;
-    cudaEvent_t e0, e1;
-    OG_CUDA_TRY(cudaMalloc((void **)&sink, 4096), return OG_ERR_CUDA);
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    int rc = OG_OK;
-    float ms = 0.f;
-    if (ogk_ffma_probe(1000, sms, sink, st) != cudaSuccess) rc = OG_ERR_CUDA;  // warm-up
-    cudaEventRecord(e0, st);
-    if (ogk_ffma_probe(iters, sms, sink, st) != cudaSuccess) rc = OG_ERR_CUDA;
-    cudaEventRecord(e1, st);
-    if (cudaEventSynchronize(e1) != cudaSuccess) rc = OG_ERR_CUDA;
-    cudaEventElapsedTime(&ms, e0, e1);
-    *ms_out = ms;
-    // grid = sms * 8 blocks x 256 threads, 8 chains, 2 flops per FFMA
-    *flops_out = (double)sms * 8.0 * 256.0 * 8.0 * 2.0 * (double)iters;
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(sink);
-    if (rc != OG_OK) og_set_error("ffma probe failed");
-    return rc;
+    int dev = 0;
+    OG_CUDA_TRY(cudaGetDevice(&dev), return OG_ERR_CUDA);
+    if (dev < 0 || dev >= 64) return OG_OK;
+    cudaMemPool_t pool;
+    {
+        std::lock_guard<std::mutex> lk(g_pool_mu);
+        pool = g_pools[dev];
+    }
+    if (pool) OG_CUDA_TRY(cudaMemPoolTrimTo(pool, 0), return OG_ERR_CUDA);
+    return OG_OK;
 }

@@ -18,7 +18,7 @@
 enum { OGC_V_FULL = 0, OGC_V_CULL, OGC_A_IN, OGC_P_IN, OGC_P_SOFT, OGC_P_OUT, OGC_FP64,
        // group-walk diagnostics: nodes per class, particles per class, batches
        OGC_CL_DROP, OGC_CL_OPEN, OGC_CL_ACCEPT, OGC_CL_GENERIC, OGC_PT_DROP, OGC_PT_SHIFT, OGC_PT_WRAP, OGC_BATCHES,
-       OGC_DIAG0, OGC_N = OGC_DIAG0 + 32 };
+       OGC_SPILLS, OGC_N };
 
 // Packed node record read by the walk: 4 x float4 + uint2.
 //   com  = (s_x, s_y, s_z, M)                 R9: fp32 rounding of the fp64 upward pass
@@ -73,9 +73,13 @@ struct og_tree {
     // walk scratch (spill stacks), allocated lazily
     void *walk_spill;
     size_t walk_spill_bytes;
-    // streams seen
+    uint32_t walk_spill_cap;   // ranges per warp in the slab
+    // stream ordering (og.h "Streams and a tree"): built = end of og_tree_build on build_stream; walked = end of
+    // the last og_shortrange_accel (recorded on its stream), waited for by the next walk and by og_tree_free
     cudaStream_t build_stream;
-    mutable cudaStream_t last_stream;
+    cudaEvent_t ev_built;
+    cudaEvent_t ev_walked;
+    mutable bool walked;
     mutable int64_t n_nodes_host;   // -1 until read back
     mutable uint32_t max_level_host;
 };
@@ -112,11 +116,10 @@ cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st);
 cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out,
                      uint64_t n_active, const float *a_old, float *acc_out, float *pot_out,
                      cudaStream_t st);
-size_t ogk_walk_spill_bytes(int sm_count);
+size_t ogk_walk_spill_bytes(int sm_count, uint32_t spill_entries);
+uint32_t ogk_walk_spill_entries(const og_params *p);
 // helpers for the active subset
 cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_perm, uint64_t n,
                              uint64_t n_active, uint64_t *keys, uint32_t *vals, uint32_t *d_status,
                              cudaStream_t st);
 cudaError_t ogk_unpack_slots(const uint64_t *keys, uint64_t n_active, uint32_t *slots, cudaStream_t st);
-// misc
-cudaError_t ogk_ffma_probe(uint64_t iters, int sm_count, float *sink, cudaStream_t st);

@@ -20,8 +20,6 @@
 // only when it has nothing left in the ring.  The split factors T, E are evaluated in registers
 // (polynomial x ex2, walk_math.cuh).  Results are written straight to the caller's order (a7
 // fused).  DESIGN.md Sec. 5 has the measured per-group counts and the instruction budget.
-//
-// k_walk_simple: one thread per target with a private stack; debugging / comparison only.
 #include "walk_math.cuh"
 
 namespace {
@@ -44,6 +42,7 @@ struct WalkArgs {
     unsigned long long *counters;
     uint32_t *spill;
     uint32_t spill_cap;        // entries per warp
+    uint32_t stack_cap;        // ranges kept in shared memory before half of them are spilled (<= GW_STACK, even)
     WalkConst c;
 };
 
@@ -72,60 +71,6 @@ __device__ __forceinline__ Target load_target(const WalkArgs &a, uint32_t k, uin
 }
 
 // -------------------------------------------------------------------------------------------
-template <bool GEOM, bool POT, bool COUNT>
-__global__ void __launch_bounds__(128)
-k_walk_simple(const __grid_constant__ WalkArgs a)
-{
-    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= a.n_active) return;
-    uint32_t out;
-    const Target t = load_target(a, k, out, GEOM);
-    unsigned long long *cnt = COUNT ? a.counters : nullptr;
-    unsigned long long c_full = 0, c_cull = 0, c_ain = 0, c_pin = 0, c_psoft = 0, c_pout = 0;
-    Accum acc = {0.f, 0.f, 0.f, 0.f};
-    uint32_t stack[176];
-    int sp = 0;
-    stack[sp++] = 0;
-    while (sp) {
-        const uint32_t j = stack[--sp];
-        const NodeRec n = load_node(a, j);
-        if (og_cull(n, t, a.c)) { ++c_cull; continue; }
-        ++c_full;
-        float dx, dy, dz, r2;
-        if (!og_open<GEOM>(n, t, a.c, dx, dy, dz, r2, cnt)) {
-            c_ain += og_monopole<POT>(n, t, a.c, dx, dy, dz, r2, acc, cnt);
-            continue;
-        }
-        const uint2 info = __ldg(a.info + j);
-        if (info.y & OG_LEAF_BIT) {
-            const uint32_t f = info.x, c = info.y & ~OG_LEAF_BIT;
-            for (uint32_t s = f; s < f + c; ++s) {
-                if (s == t.slot) continue;
-                const int kind = og_pair<POT>(__ldg(a.spos + s), __ldg(a.sh + s), t, a.c, acc, cnt);
-                if (kind == 0) ++c_pout; else { ++c_pin; if (kind == 2) ++c_psoft; }
-            }
-        } else {
-            for (uint32_t ch = 0; ch < info.y; ++ch) {
-                if (sp >= 176) { atomicOr(a.status, OG_DEV_STACK_OVERFLOW); break; }
-                stack[sp++] = info.x + info.y - 1 - ch;
-            }
-        }
-    }
-    a.acc_out[3 * (size_t)out] = acc.ax;
-    a.acc_out[3 * (size_t)out + 1] = acc.ay;
-    a.acc_out[3 * (size_t)out + 2] = acc.az;
-    if (POT) a.pot_out[out] = acc.pot;
-    if (COUNT) {
-        atomicAdd(&a.counters[OGC_V_FULL], c_full);
-        atomicAdd(&a.counters[OGC_V_CULL], c_cull);
-        atomicAdd(&a.counters[OGC_A_IN], c_ain);
-        atomicAdd(&a.counters[OGC_P_IN], c_pin);
-        atomicAdd(&a.counters[OGC_P_SOFT], c_psoft);
-        atomicAdd(&a.counters[OGC_P_OUT], c_pout);
-    }
-}
-
-// -------------------------------------------------------------------------------------------
 #ifndef OG_GW_WARPS
 #define OG_GW_WARPS 8
 #endif
@@ -144,12 +89,16 @@ k_walk_simple(const __grid_constant__ WalkArgs a)
 #ifndef OG_GW_STACK
 #define OG_GW_STACK 256
 #endif
+#ifndef OG_CONSUME_PIPELINED
+#define OG_CONSUME_PIPELINED 0
+#endif
 constexpr int GW_WARPS = OG_GW_WARPS;           // warps per block
 constexpr int GW_THREADS = GW_WARPS * 32;
 constexpr int GW_STACK = OG_GW_STACK;         // node-range stack entries per warp in shared memory
-constexpr int GW_SPILL = GW_STACK / 2;        // entries moved to / from global memory at a time
 constexpr int GW_PLIST = 64;          // particle-range list entries per warp
 constexpr int GW_NSEG = OG_GW_NSEG;            // 32-source segments in the per-warp source ring (power of two)
+
+constexpr uint32_t GW_DUMMY = GW_NSEG * 32;   // ring slot of a source at (1e18, 1e18, 1e18) with mass 0
 
 #define SEG_PART 2u      // particle segment (else node segment); only the counters care
 
@@ -158,12 +107,16 @@ constexpr int GW_NSEG = OG_GW_NSEG;            // 32-source segments in the per-
 // with slot j of the segment.  Each lane later walks its OWN set bits (per-lane compaction), so a lane
 // is idle only when its list is shorter than the longest one of the buffered window.
 struct __align__(16) WarpSmem {
-    float4 ring_pos[GW_NSEG * 32];      // (x', y', z', G m): pre-shifted to the group's periodic image
-    float ring_h[GW_NSEG * 32];         // softening length of the source (0 for nodes)
+    float4 ring_pos[GW_NSEG * 32 + 1];  // (x', y', z', G m): pre-shifted to the group's periodic image; + the dummy slot
+    float ring_h[GW_NSEG * 32 + 4];     // softening length of the source (0 for nodes)
     uint32_t W[GW_NSEG][32];
-    float4 xn_com[32], xn_aux[32], xn_cel[32];   // undecided nodes: (s', GM), (lhs, near2, cull2, band), (c', l)
+    // undecided nodes of a batch, in pairs (for the packed test loop): pair p = nodes 2p, 2p + 1 of the batch's
+    // undecided nodes in lane order; xq[p] = (x0, x1, y0, y1), (z0, z1, cull2_0, cull2_1),
+    // (lhs_0 (1 - band), lhs_1 (1 - band), lhs_0 (1 + band), lhs_1 (1 + band)), (near2_0, near2_1, mask_0, mask_1)
+    float4 xq[16][4];
+    float4 xn_cel[32];                  // (c', l) per undecided node (guards, exact path)
     float xn_hm2[32];                   // h_max^2
-    uint32_t xn_idx[32];
+    uint32_t xn_u[32];                  // undecided node: node index; node accepted by all: its target mask
     uint32_t seg_flags[GW_NSEG];
     uint32_t st_start[GW_STACK], st_cnt[GW_STACK], st_mask[GW_STACK];
     uint32_t pl_start[GW_PLIST], pl_cnt[GW_PLIST], pl_mask[GW_PLIST];
@@ -173,6 +126,21 @@ struct __align__(16) WarpSmem {
 __device__ __forceinline__ void or_if(uint32_t &w, const uint32_t bit, const bool p)
 {
     asm("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %2, 0;\n\t@q or.b32 %0, %0, %1;\n\t}" : "+r"(w) : "r"(bit), "r"((uint32_t)p));
+}
+
+// index of the most significant set bit, 0xffffffff if x == 0 (one FLO; __ffs costs BREV + FLO)
+__device__ __forceinline__ uint32_t og_bfind(uint32_t x)
+{
+    uint32_t r;
+    asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+    return r;
+}
+// x << n with n >= 32 giving 0 (PTX shl clamps; the C++ operator is undefined there)
+__device__ __forceinline__ uint32_t og_shl(uint32_t x, uint32_t n)
+{
+    uint32_t r;
+    asm("shl.b32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(n));
+    return r;
 }
 
 __device__ __forceinline__ uint32_t lanemask_lt()
@@ -252,8 +220,8 @@ enum { CL_DROP = 0, CL_OPEN = 1, CL_ACCEPT = 2, CL_GENERIC = 3 };
 // s >= L/2), else sc holds s itself and the lanes wrap.
 template <bool GEOM>
 __device__ __forceinline__ int classify_node(const float4 n0, float R, float ng, float l, const GroupInfo &g,
-                                             const WalkConst &c, float4 &sc, float4 &aux, bool &shifted,
-                                             float &kx, float &ky, float &kz)
+                                             const WalkConst &c, float4 &sc, float &lhs, float &near2, float &cull2,
+                                             bool &shifted, float &kx, float &ky, float &kz)
 {
     kx = rintf((n0.x - g.gcx) * c.invL); ky = rintf((n0.y - g.gcy) * c.invL); kz = rintf((n0.z - g.gcz) * c.invL);
     const float adx = fabsf(fmaf(-c.L, kx, n0.x - g.gcx)), ady = fabsf(fmaf(-c.L, ky, n0.y - g.gcy)),
@@ -263,11 +231,11 @@ __device__ __forceinline__ int classify_node(const float4 n0, float R, float ng,
     const float rmin2 = fmaf(nz, nz, fmaf(ny, ny, nx * nx));
     const float rmax2 = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
     const float rc = c.cull_r + R;
-    const float cull2 = rc * rc;
+    cull2 = rc * rc;
     if (rmin2 > cull2) return CL_DROP;
     const float l2 = l * l;
     const float GM = c.G * n0.w;
-    float lhs, rhs_max, rhs_min;
+    float rhs_max, rhs_min;
     if (GEOM) {
         lhs = l2; rhs_max = c.theta2 * rmax2; rhs_min = c.theta2 * rmin2;
     } else {
@@ -282,12 +250,13 @@ __device__ __forceinline__ int classify_node(const float4 n0, float R, float ng,
               (ky == 0.0f || (ky == 1.0f && n0.y >= hL)) && (kz == 0.0f || (kz == 1.0f && n0.z >= hL));
     if (shifted) sc = make_float4(fmaf(-c.L, kx, n0.x), fmaf(-c.L, ky, n0.y), fmaf(-c.L, kz, n0.z), GM);
     else sc = make_float4(n0.x, n0.y, n0.z, GM);
-    const float ng2 = ng * ng;
-    if (lhs < rhs_min * (1.0f - OG_GM) && rmin2 > fmaxf(ng2, g.hmax2) * (1.0f + OG_GM)) {
+    // no guard (R15 / R16) can fire for a target farther than this from s: ng covers the guard box and the
+    // node's h_max, the group's largest own h covers every target's softening length
+    near2 = fmaxf(ng * ng, g.hmax2) * (1.0f + OG_GM);
+    if (lhs < rhs_min * (1.0f - OG_GM) && rmin2 > near2) {
         if (rmin2 > c.rcut2 * (1.0f + OG_GM)) return CL_DROP;
         return CL_ACCEPT;
     }
-    aux = make_float4(lhs, ng2 * (1.0f + OG_GM), cull2, OG_BAND * lhs);
     return CL_GENERIC;
 }
 
@@ -352,106 +321,174 @@ __device__ __noinline__ float4 pair_exact(const float4 q, const float hj, const 
 }
 
 // Position of a lane in the source ring: `nxt` = next segment (monotone counter) whose word the lane will
-// load, `cur` = bits of segment nxt - 1 it has not evaluated yet, `base` = ring slot of that segment's
-// first source.
+// take, `cur` = bits of segment nxt - 1 it has not evaluated yet, `base` = ring slot of that segment's
+// first source, `nw` = the word of segment nxt, loaded ahead (valid while nxt < head).
 struct LanePos {
-    uint32_t nxt, cur, base, part;   // part: the segment holds particles (counters only)
+    uint32_t nxt, cur, base, nw;
 };
 
-// Evaluates ring sources until every lane has finished all segments < target (target <= head, the number
-// of segments produced so far).  Every lane walks the set bits of its own words, two sources per
-// iteration (two independent dependency chains).  Newtonian monopole x split factor in the loop (R21);
-// a source that is within OG_BAND of r_cut or closer than the largest softening length of the whole
-// particle set goes to pair_exact.  Returns the number of segments all lanes have finished.
-template <bool POT, bool COUNT, bool WRAP, bool HLOOK>
-__device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, const uint32_t target, LanePos &lp,
-                                            const Target &t, const float hmax2g, const WalkConst &c, Accum &acc,
-                                            const uint32_t lane, unsigned long long *cnt, LaneCount &lc)
+// Per-target accumulators of the group walk: two partial sums per component (the two source chains of the
+// consume loop accumulate side by side in one register pair); pot holds +sum(G m E / r), negated at the end.
+struct Accum2 {
+    f32x2 ax, ay, az, pot;
+};
+
+__device__ __forceinline__ void acc2_add(f32x2 &v, float d)
 {
-    uint32_t it = 0u;
-    for (;;) {
-        if (lp.cur == 0u && lp.nxt < head) {
-            const uint32_t sl = lp.nxt & (GW_NSEG - 1);
-            lp.cur = w.W[sl][lane];
-            lp.base = sl * 32u;
-            if (COUNT) lp.part = w.seg_flags[sl] & SEG_PART;
-            ++lp.nxt;
+    float a, b;
+    upk2(v, a, b);
+    v = pk2(a + d, b);
+}
+
+// Takes the next two sources of the lane's own list: moves on to the next produced segment if the current
+// word is used up (its word was loaded ahead; the one after it is requested now), then extracts the lowest
+// and the highest set bit of the word (two independent FLO; the order within a segment is free).  A lane
+// without a (second) source gets the far-away dummy slot: beyond r_cut, nothing happens.
+__device__ __forceinline__ void take_two(WarpSmem &w, LanePos &lp, const uint32_t head, const uint32_t lane,
+                                         uint32_t &e0, uint32_t &e1)
+{
+    if (lp.cur == 0u && lp.nxt < head) {
+        lp.cur = lp.nw;
+        lp.base = (lp.nxt & (GW_NSEG - 1)) * 32u;
+        ++lp.nxt;
+        lp.nw = w.W[lp.nxt & (GW_NSEG - 1)][lane];   // (a stale word if nxt == head: reloaded at the next call)
+    }
+    const uint32_t cur = lp.cur;
+    const uint32_t low = cur & (0u - cur);
+    const uint32_t ilo = og_bfind(low), ihi = og_bfind(cur);     // 0xffffffff if there is none
+    e0 = (cur != 0u) ? lp.base + ilo : GW_DUMMY;
+    e1 = (ihi != ilo) ? lp.base + ihi : GW_DUMMY;
+    lp.cur = (cur ^ low) & ~og_shl(1u, ihi);
+}
+
+// Two sources q0, q1 (ring slots e0, e1) against the lane's target, evaluated as ONE chain of packed fp32
+// pairs (FFMA2 / FMUL2, walk_math.cuh).  Newtonian monopole x split factor (R21); a source that is within
+// OG_BAND of r_cut or closer than the largest softening length of the whole particle set goes to pair_exact.
+template <bool POT, bool COUNT, bool WRAP, bool HLOOK>
+__device__ __forceinline__ void eval_two(WarpSmem &w, const float4 q0, const float4 q1, const uint32_t e0, const uint32_t e1,
+                                         const Target &t, const float hmax2g, const WalkConst &c, Accum2 &acc,
+                                         unsigned long long *cnt, LaneCount &lc)
+{
+    const bool v0 = e0 != GW_DUMMY, v1 = e1 != GW_DUMMY;
+    float dx0 = q0.x - t.x, dy0 = q0.y - t.y, dz0 = q0.z - t.z;
+    float dx1 = q1.x - t.x, dy1 = q1.y - t.y, dz1 = q1.z - t.z;
+    if (WRAP) {
+        dx0 = og_wrap(dx0, c); dy0 = og_wrap(dy0, c); dz0 = og_wrap(dz0, c);
+        dx1 = og_wrap(dx1, c); dy1 = og_wrap(dy1, c); dz1 = og_wrap(dz1, c);
+    }
+    const f32x2 dx = pk2(dx0, dx1), dy = pk2(dy0, dy1), dz = pk2(dz0, dz1);
+    const f32x2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+    float r20, r21;
+    upk2(r2, r20, r21);
+    // fast: strictly inside the cutoff band and not softened: anything closer than the largest h of the
+    // whole particle set (h_max of the root) takes the exact path.  HLOOK (the 8-targets-per-warp kernel,
+    // used for sparse active subsets, where a multi-species zoom has h comparable to r_cut): the source's
+    // own h is looked up below that bound (nodes carry h = 0: R16 keeps accepted nodes outside the
+    // target's own h).
+    bool fast0, fast1;
+    if (HLOOK) {
+        bool soft0 = r20 < hmax2g, soft1 = r21 < hmax2g;
+        float hj0 = 0.0f, hj1 = 0.0f;
+        if ((!WRAP || v0) && soft0) hj0 = w.ring_h[e0];
+        if ((!WRAP || v1) && soft1) hj1 = w.ring_h[e1];
+        const float hh0 = fmaxf(t.h, hj0), hh1 = fmaxf(t.h, hj1);
+        soft0 = soft0 && r20 < hh0 * hh0 * (1.0f + OG_BAND);
+        soft1 = soft1 && r21 < hh1 * hh1 * (1.0f + OG_BAND);
+        fast0 = (!WRAP || v0) && r20 < c.rcut2_lo && !soft0;
+        fast1 = (!WRAP || v1) && r21 < c.rcut2_lo && !soft1;
+    } else {
+        // (the wrapped distance of the dummy slot is arbitrary: WRAP keeps the validity predicates)
+        fast0 = (!WRAP || v0) && r20 < c.rcut2_lo && r20 >= hmax2g;
+        fast1 = (!WRAP || v1) && r21 < c.rcut2_lo && r21 >= hmax2g;
+    }
+    const bool slow0 = (!WRAP || v0) && !fast0 && r20 < c.rcut2_hi;
+    const bool slow1 = (!WRAP || v1) && !fast1 && r21 < c.rcut2_hi;
+    {
+        // 1 / r is replaced by 0 for a source that is not "fast" (masked, beyond r_cut, softened or exact path):
+        // then r = w = 0, T = E = exp(..) <= 1 and the force and potential terms vanish, all finite (ring slots
+        // hold finite values only); fast sources have hmax2g <= r^2 < r_cut^2, inside the range of og_split2
+        const f32x2 ri = pk2(fast0 ? og_rsqrt(r20) : 0.0f, fast1 ? og_rsqrt(r21) : 0.0f);
+        float ri0, ri1;
+        upk2(ri, ri0, ri1);
+        f32x2 T, E;
+        og_split2(mul2(r2, ri), r2, c, T, E);
+        const f32x2 gr = pk2(q0.w * ri0, q1.w * ri1);
+        const f32x2 f = mul2(mul2(gr, T), mul2(ri, ri));
+        acc.ax = fma2(f, dx, acc.ax); acc.ay = fma2(f, dy, acc.ay); acc.az = fma2(f, dz, acc.az);
+        if (POT) acc.pot = fma2(gr, E, acc.pot);
+    }
+    int k0 = fast0 ? 1 : 0, k1 = fast1 ? 1 : 0;
+    if (slow0 | slow1) {
+        if (slow0) {
+            const float4 d = pair_exact<POT>(q0, w.ring_h[e0], t, c, cnt, k0);
+            acc2_add(acc.ax, d.x); acc2_add(acc.ay, d.y); acc2_add(acc.az, d.z); acc2_add(acc.pot, -d.w);
         }
-        uint32_t cur = lp.cur;
-        const bool v0 = cur != 0u;
-        const uint32_t e0 = lp.base + ((__ffs(cur) - 1) & 31);
-        cur &= cur - 1u;
-        const bool v1 = cur != 0u;
-        const uint32_t e1 = lp.base + ((__ffs(cur) - 1) & 31);
-        cur &= cur - 1u;
-        lp.cur = cur;
-        const float4 q0 = w.ring_pos[e0], q1 = w.ring_pos[e1];
-        float dx0 = q0.x - t.x, dy0 = q0.y - t.y, dz0 = q0.z - t.z;
-        float dx1 = q1.x - t.x, dy1 = q1.y - t.y, dz1 = q1.z - t.z;
-        if (WRAP) {
-            dx0 = og_wrap(dx0, c); dy0 = og_wrap(dy0, c); dz0 = og_wrap(dz0, c);
-            dx1 = og_wrap(dx1, c); dy1 = og_wrap(dy1, c); dz1 = og_wrap(dz1, c);
-        }
-        const float r20 = fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0));
-        const float r21 = fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1));
-        // fast: strictly inside the cutoff band and not softened: anything closer than the largest h of the
-        // whole particle set (h_max of the root) takes the exact path.  HLOOK (the 8-targets-per-warp kernel,
-        // used for sparse active subsets, where a multi-species zoom has h comparable to r_cut): the source's
-        // own h is looked up below that bound (nodes carry h = 0: R16 keeps accepted nodes outside the
-        // target's own h).
-        bool fast0, fast1;
-        if (HLOOK) {
-            bool soft0 = r20 < hmax2g, soft1 = r21 < hmax2g;
-            float hj0 = 0.0f, hj1 = 0.0f;
-            if (v0 && soft0) hj0 = w.ring_h[e0];
-            if (v1 && soft1) hj1 = w.ring_h[e1];
-            const float hh0 = fmaxf(t.h, hj0), hh1 = fmaxf(t.h, hj1);
-            soft0 = soft0 && r20 < hh0 * hh0 * (1.0f + OG_BAND);
-            soft1 = soft1 && r21 < hh1 * hh1 * (1.0f + OG_BAND);
-            fast0 = v0 && r20 < c.rcut2_lo && !soft0;
-            fast1 = v1 && r21 < c.rcut2_lo && !soft1;
-        } else {
-            fast0 = v0 && r20 < c.rcut2_lo && r20 >= hmax2g;
-            fast1 = v1 && r21 < c.rcut2_lo && r21 >= hmax2g;
-        }
-        const bool slow0 = v0 && !fast0 && r20 < c.rcut2_hi;
-        const bool slow1 = v1 && !fast1 && r21 < c.rcut2_hi;
-        {
-            const float r2a = fmaxf(r20, 1.0e-20f), r2b = fmaxf(r21, 1.0e-20f);
-            const float ria = og_rsqrt(r2a), rib = og_rsqrt(r2b);
-            float Ta, Ea, Tb, Eb;
-            og_split(r2a * ria, r2a, c, Ta, Ea);
-            og_split(r2b * rib, r2b, c, Tb, Eb);
-            const float gra = (fast0 ? q0.w : 0.0f) * ria, grb = (fast1 ? q1.w : 0.0f) * rib;
-            const float fa = gra * Ta * (ria * ria), fb = grb * Tb * (rib * rib);
-            acc.ax = fmaf(fa, dx0, acc.ax); acc.ay = fmaf(fa, dy0, acc.ay); acc.az = fmaf(fa, dz0, acc.az);
-            acc.ax = fmaf(fb, dx1, acc.ax); acc.ay = fmaf(fb, dy1, acc.ay); acc.az = fmaf(fb, dz1, acc.az);
-            if (POT) { acc.pot = fmaf(-gra, Ea, acc.pot); acc.pot = fmaf(-grb, Eb, acc.pot); }
-        }
-        int k0 = fast0 ? 1 : 0, k1 = fast1 ? 1 : 0;
-        if (slow0 | slow1) {
-            if (slow0) {
-                const float4 d = pair_exact<POT>(q0, w.ring_h[e0], t, c, cnt, k0);
-                acc.ax += d.x; acc.ay += d.y; acc.az += d.z; acc.pot += d.w;
-            }
-            if (slow1) {
-                const float4 d = pair_exact<POT>(q1, w.ring_h[e1], t, c, cnt, k1);
-                acc.ax += d.x; acc.ay += d.y; acc.az += d.z; acc.pot += d.w;
-            }
-        }
-        if (COUNT) {
-            if (lp.part) {
-                lc.pin += (k0 != 0) + (k1 != 0); lc.psoft += (k0 == 2) + (k1 == 2);
-                lc.pout += (v0 && k0 == 0) + (v1 && k1 == 0);
-            } else {
-                lc.ain += (k0 != 0) + (k1 != 0);
-            }
-        }
-        if ((++it & 1u) == 0u) {   // the exit test (a warp reduction) every second iteration
-            const uint32_t done = __reduce_min_sync(0xffffffffu, (cur == 0u) ? lp.nxt : lp.nxt - 1u);
-            if (done >= target) return done;
+        if (slow1) {
+            const float4 d = pair_exact<POT>(q1, w.ring_h[e1], t, c, cnt, k1);
+            acc2_add(acc.ax, d.x); acc2_add(acc.ay, d.y); acc2_add(acc.az, d.z); acc2_add(acc.pot, -d.w);
         }
     }
+    if (COUNT) {
+        const bool part0 = (w.seg_flags[(e0 >> 5) & (GW_NSEG - 1)] & SEG_PART) != 0u;
+        const bool part1 = (w.seg_flags[(e1 >> 5) & (GW_NSEG - 1)] & SEG_PART) != 0u;
+        if (v0) { if (part0) { lc.pin += (k0 != 0); lc.psoft += (k0 == 2); lc.pout += (k0 == 0); } else lc.ain += (k0 != 0); }
+        if (v1) { if (part1) { lc.pin += (k1 != 0); lc.psoft += (k1 == 2); lc.pout += (k1 == 0); } else lc.ain += (k1 != 0); }
+    }
+}
+
+// Evaluates ring sources until every lane has finished all segments < target (tail <= target <= head; head =
+// segments produced so far, tail = segments every lane had finished before).  Every lane walks the set bits
+// of its own words, two sources per step; lanes with shorter lists run ahead into the segments >= target.
+// The number of steps is known in advance (a word of k bits takes max(1, ceil(k / 2)) steps), so the loop has
+// no exit test, and the sources of the next step are taken and loaded while the current pair is evaluated
+// (unrolled by two so that the two pairs alternate between two register sets).  Returns the number of
+// segments all lanes have finished.
+template <bool POT, bool COUNT, bool WRAP, bool HLOOK>
+__device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, const uint32_t tail, const uint32_t target,
+                                            LanePos &lp, const Target &t, const float hmax2g, const WalkConst &c,
+                                            Accum2 &acc, const uint32_t lane, unsigned long long *cnt, LaneCount &lc)
+{
+    // the word in progress is segment nxt - 1: it counts only if the lane is not already past the target
+    uint32_t need = (lp.nxt <= target) ? (uint32_t)(__popc(lp.cur) + 1) >> 1 : 0u;
+    for (uint32_t sg = tail; sg < target; ++sg) {
+        const uint32_t ww = w.W[sg & (GW_NSEG - 1)][lane];
+        const uint32_t k = max((uint32_t)(__popc(ww) + 1) >> 1, 1u);
+        if (sg >= lp.nxt) need += k;
+    }
+    const uint32_t steps = __reduce_max_sync(0xffffffffu, need);
+#if OG_CONSUME_PIPELINED
+    if (steps != 0u) {
+        lp.nw = w.W[lp.nxt & (GW_NSEG - 1)][lane];
+        uint32_t e0, e1, f0, f1;
+        take_two(w, lp, head, lane, e0, e1);
+        float4 q0 = w.ring_pos[e0], q1 = w.ring_pos[e1], p0, p1;
+        uint32_t it = 1u;
+        for (; it + 1u < steps; it += 2u) {
+            take_two(w, lp, head, lane, f0, f1);
+            p0 = w.ring_pos[f0]; p1 = w.ring_pos[f1];
+            eval_two<POT, COUNT, WRAP, HLOOK>(w, q0, q1, e0, e1, t, hmax2g, c, acc, cnt, lc);
+            take_two(w, lp, head, lane, e0, e1);
+            q0 = w.ring_pos[e0]; q1 = w.ring_pos[e1];
+            eval_two<POT, COUNT, WRAP, HLOOK>(w, p0, p1, f0, f1, t, hmax2g, c, acc, cnt, lc);
+        }
+        if (it < steps) {
+            take_two(w, lp, head, lane, f0, f1);
+            p0 = w.ring_pos[f0]; p1 = w.ring_pos[f1];
+            eval_two<POT, COUNT, WRAP, HLOOK>(w, q0, q1, e0, e1, t, hmax2g, c, acc, cnt, lc);
+            q0 = p0; q1 = p1; e0 = f0; e1 = f1;
+        }
+        eval_two<POT, COUNT, WRAP, HLOOK>(w, q0, q1, e0, e1, t, hmax2g, c, acc, cnt, lc);
+    }
+#else
+    lp.nw = w.W[lp.nxt & (GW_NSEG - 1)][lane];
+    for (uint32_t it = 0u; it < steps; ++it) {
+        uint32_t e0, e1;
+        take_two(w, lp, head, lane, e0, e1);
+        const float4 q0 = w.ring_pos[e0], q1 = w.ring_pos[e1];
+        eval_two<POT, COUNT, WRAP, HLOOK>(w, q0, q1, e0, e1, t, hmax2g, c, acc, cnt, lc);
+    }
+#endif
+    return __reduce_min_sync(0xffffffffu, (lp.cur == 0u) ? lp.nxt : lp.nxt - 1u);
 }
 
 // G = targets per warp (32, or 8 for sparse active subsets), K = 32 / G lanes per target: lane = s * G + t
@@ -477,11 +514,14 @@ k_walk_group(const __grid_constant__ WalkArgs a)
     unsigned long long *cnt = COUNT ? a.counters : nullptr;
     uint32_t *sp_start = a.spill + (size_t)(blockIdx.x * GW_WARPS + wid) * 3 * a.spill_cap;
     uint32_t *sp_cnt = sp_start + a.spill_cap, *sp_mask = sp_cnt + a.spill_cap;
+    const uint32_t half = a.stack_cap >> 1;   // ranges moved to / from the global slab at a time
     // largest softening length of the whole particle set = h_max of the root (R16 / R19 can only matter below it)
     const float hroot = __ldg(a.lo).w;
-    const float hmax2g = hroot * hroot * (1.0f + OG_BAND);
+    // (> 0 even if no particle is softened: a coincident source, r = 0, must take the exact path)
+    const float hmax2g = fmaxf(hroot * hroot * (1.0f + OG_BAND), 1.0e-30f);
     // stale ring slots are read (and masked out) by lanes that have nothing to do: keep them finite
     for (int i = lane; i < GW_NSEG * 32; i += 32) { w.ring_pos[i] = make_float4(0.f, 0.f, 0.f, 0.f); w.ring_h[i] = 0.f; }
+    if (lane == 0) { w.ring_pos[GW_DUMMY] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.f); w.ring_h[GW_DUMMY] = 0.f; }
     __syncwarp();
 
     for (;;) {
@@ -521,12 +561,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
         // lanes whose target is the same sorted slot (duplicates in active_idx; the mirrored tail lanes)
         const uint32_t peers = __match_any_sync(0xffffffffu, t.slot) & TMASK;   // as a target mask
         const float hi2 = t.h * t.h;
-        const float hi2m = hi2 * (1.0f + OG_GM);   // own softening guard threshold (R16), padded
-        Accum acc = {0.f, 0.f, 0.f, 0.f};
+        Accum2 acc2 = {0ull, 0ull, 0ull, 0ull};
         LaneCount lc = {0, 0, 0, 0, 0, 0};
-        // diag (OG_COUNT): groups binned by their largest half extent relative to r_cut
-        uint32_t dg_gen = 0, dg_bat = 0;
-        const long long dg_t0 = COUNT ? clock64() : 0;
         int top = 0, pl_top = 0;
         uint32_t pl_items = 0, spill_n = 0;
         uint32_t head = 0, tail = 0;          // ring: segments produced / finished by all lanes
@@ -540,7 +576,7 @@ k_walk_group(const __grid_constant__ WalkArgs a)
         }
         for (;;) {
             if (top == 0 && spill_n > 0) {  // reload spilled entries
-                const uint32_t m = min(spill_n, (uint32_t)GW_SPILL);
+                const uint32_t m = min(spill_n, half);
                 for (uint32_t i = lane; i < m; i += 32) {
                     w.st_start[i] = sp_start[spill_n - m + i];
                     w.st_cnt[i] = sp_cnt[spill_n - m + i];
@@ -557,8 +593,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 // ring full: free at least half of it; finishing: drain it
                 __syncwarp();
                 const uint32_t target = fin ? head : tail + GW_NSEG / 2;
-                tail = anywrap ? consume<POT, COUNT, true, (G < 32)>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc)
-                               : consume<POT, COUNT, false, (G < 32)>(w, head, target, lp, t, hmax2g, c, acc, lane, cnt, lc);
+                tail = anywrap ? consume<POT, COUNT, true, (G < 32)>(w, head, tail, target, lp, t, hmax2g, c, acc2, lane, cnt, lc)
+                               : consume<POT, COUNT, false, (G < 32)>(w, head, tail, target, lp, t, hmax2g, c, acc2, lane, cnt, lc);
                 __syncwarp();
             }
             if (fin) break;
@@ -569,6 +605,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 uint32_t first = 0, meta = 0;
                 int cls = CL_DROP;
                 bool shifted = true;
+                float4 sc = make_float4(0.f, 0.f, 0.f, 0.f), cel = sc;
+                float lhs = 0.f, near2 = 0.f, cull2 = 0.f, hm2 = 0.f;
                 if (lane < total) {
                     const uint4 *rp = a.rec + 3 * (size_t)item;
                     const uint4 r0 = __ldg(rp), n1 = __ldg(rp + 1), r2 = __ldg(rp + 2);
@@ -576,38 +614,51 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     const float4 n2 = make_float4(__uint_as_float(r2.x), __uint_as_float(r2.y), __uint_as_float(r2.z), __uint_as_float(r2.w));
                     first = n1.z; meta = n1.w;
                     const float l = c.L * __uint_as_float((127u - (meta >> 27)) << 23);   // L / 2^level, exact
-                    float4 sc, aux;
                     float kx, ky, kz;
-                    cls = classify_node<GEOM>(n0, __uint_as_float(n1.x), __uint_as_float(n1.y), l, g, c, sc, aux,
-                                              shifted, kx, ky, kz);
-                    if (cls >= CL_ACCEPT) {
-                        w.ring_pos[slot0 + lane] = sc;
-                        w.ring_h[slot0 + lane] = 0.0f;
-                    }
+                    cls = classify_node<GEOM>(n0, __uint_as_float(n1.x), __uint_as_float(n1.y), l, g, c, sc, lhs, near2,
+                                              cull2, shifted, kx, ky, kz);
                     if (cls == CL_GENERIC) {
-                        w.xn_com[lane] = sc; w.xn_aux[lane] = aux;
                         // cell centre in the same periodic image as sc (exact for k in {0, 1}, see classify_node)
-                        w.xn_cel[lane] = shifted ? make_float4(fmaf(-c.L, kx, n2.x), fmaf(-c.L, ky, n2.y),
-                                                               fmaf(-c.L, kz, n2.z), l)
-                                                 : make_float4(n2.x, n2.y, n2.z, l);
-                        w.xn_hm2[lane] = n2.w * n2.w;
-                        w.xn_idx[lane] = item;
+                        cel = shifted ? make_float4(fmaf(-c.L, kx, n2.x), fmaf(-c.L, ky, n2.y), fmaf(-c.L, kz, n2.z), l)
+                                      : make_float4(n2.x, n2.y, n2.z, l);
+                        hm2 = n2.w * n2.w;
                     }
                 }
                 const uint32_t bA = __ballot_sync(0xffffffffu, cls == CL_ACCEPT);
                 const uint32_t bX = __ballot_sync(0xffffffffu, cls == CL_GENERIC);
                 const uint32_t bW = __ballot_sync(0xffffffffu, cls >= CL_ACCEPT && !shifted);
                 anywrap |= bW != 0u;
-                // Mt: bit j = my target is in the mask of the node lane j holds
-                const uint32_t Mt = transpose32((cls >= CL_ACCEPT) ? imask * REP : 0u, lane);
+                // ring slots of the segment: the undecided nodes first (in lane order), then the nodes every
+                // target accepts; rX also numbers the undecided nodes in the staging arrays
+                const uint32_t nX = __popc(bX), nA = __popc(bA);
+                const uint32_t rX = __popc(bX & lt), rA = nX + __popc(bA & lt);
+                if (cls == CL_GENERIC) {
+                    w.ring_pos[slot0 + rX] = sc;
+                    w.ring_h[slot0 + rX] = 0.0f;
+                    float *f = &w.xq[rX >> 1][0].x + (rX & 1u);
+                    f[0] = sc.x; f[2] = sc.y; f[4] = sc.z; f[6] = cull2;
+                    f[8] = lhs * (1.0f - OG_BAND); f[10] = lhs * (1.0f + OG_BAND);
+                    f[12] = near2; f[14] = __uint_as_float(imask);
+                    if ((rX & 1u) == 0u && rX + 1u == nX) {   // odd count: the other half of the last pair tests nothing
+                        f[1] = 0.f; f[3] = 0.f; f[5] = 0.f; f[7] = -1.0f; f[9] = 0.f; f[11] = 0.f; f[13] = 0.f; f[15] = 0.f;
+                    }
+                    w.xn_cel[rX] = cel; w.xn_hm2[rX] = hm2; w.xn_u[rX] = item;
+                }
+                if (cls == CL_ACCEPT) {
+                    w.ring_pos[slot0 + rA] = sc;
+                    w.ring_h[slot0 + rA] = 0.0f;
+                    w.xn_u[rA] = imask;
+                }
                 __syncwarp();
+                // MtA: bit j = my target is in the mask of the all-accepted node in ring slot j
+                uint32_t MtA = 0u;
+                if (bA != 0u) MtA = transpose32((lane >= nX && lane < nX + nA) ? w.xn_u[lane] * REP : 0u, lane);
                 if (COUNT) {   // group-level outcomes counted as the per-target visits they stand for
                     const uint32_t bO = __ballot_sync(0xffffffffu, cls == CL_OPEN);
                     if (lane == 0) {
                         atomicAdd(&a.counters[OGC_CL_OPEN], (unsigned long long)__popc(bO));
                         atomicAdd(&a.counters[OGC_CL_ACCEPT], (unsigned long long)__popc(bA));
                         atomicAdd(&a.counters[OGC_CL_GENERIC], (unsigned long long)__popc(bX));
-                        dg_gen += __popc(bX); ++dg_bat;
                         atomicAdd(&a.counters[OGC_CL_DROP], (unsigned long long)(total - __popc(bA | bX | bO)));
                         atomicAdd(&a.counters[OGC_BATCHES], 1ull);
                     }
@@ -618,41 +669,37 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                         if (sl == 0u && (mj & mybit) && cj == CL_DROP) ++lc.cull;
                     }
                 }
-                // Undecided nodes: every lane tests every staged node (broadcast LDS) branch-free on
-                // (s', GM, lhs, near2, cull2, band): culled / opens / accepts / needs the guards.  The
-                // few lanes of the last kind then evaluate the guards R15 / R16 from the staged cell, and
-                // anything within the band of a threshold takes the exact out-of-line decision.
+                // Undecided nodes: every lane (G = 32; for G < 32 slice s of a target takes the pairs = s mod K)
+                // tests the staged nodes two at a time as packed fp32 pairs (broadcast LDS.128), branch-free:
+                // not in the mask or beyond r_cut + R of the node / opens / accepts / needs the guards.  The few
+                // lanes of the last kind then evaluate the guards R15 / R16 from the staged cell, and anything
+                // within the band of a threshold takes the exact out-of-line decision.
                 uint32_t accw = 0u, myopen = 0u;
                 if (bX != 0u) {
                     const bool xwrap = (bX & bW) != 0u;
                     uint32_t openw = 0u, sloww = 0u;
-                    // G = 32: every lane tests every node (uniform loop); G < 32: slice s of a target tests the
-                    // nodes of the slots = s (mod K), so K different nodes are tested per step
-                    uint32_t rem = bX & myslots;
-                    while (G == 32 ? (rem != 0u) : __any_sync(0xffffffffu, rem != 0u)) {   // two nodes per iteration
-                        const bool one = rem != 0u;
-                        const int j0 = (__ffs(rem) - 1) & 31;
-                        rem &= rem - 1u;
-                        const bool two = rem != 0u;
-                        const int j1 = two ? __ffs(rem) - 1 : j0;
-                        rem &= rem - 1u;
-                        const float4 s0 = w.xn_com[j0], s1 = w.xn_com[j1];
-                        const float4 x0 = w.xn_aux[j0], x1 = w.xn_aux[j1];
-                        float dx0 = s0.x - t.x, dy0 = s0.y - t.y, dz0 = s0.z - t.z;
-                        float dx1 = s1.x - t.x, dy1 = s1.y - t.y, dz1 = s1.z - t.z;
+                    const uint32_t np = (nX + 1u) >> 1;
+                    const f32x2 tx2 = bc2(t.x), ty2 = bc2(t.y), tz2 = bc2(t.z), A2 = bc2(GEOM ? c.theta2 : t.A);
+#pragma unroll 2
+                    for (uint32_t p = sl; p < np; p += (uint32_t)K) {
+                        const float4 a0 = w.xq[p][0], a1 = w.xq[p][1], a2 = w.xq[p][2], a3 = w.xq[p][3];
+                        f32x2 dx = sub2(pk2(a0.x, a0.y), tx2), dy = sub2(pk2(a0.z, a0.w), ty2), dz = sub2(pk2(a1.x, a1.y), tz2);
                         if (xwrap) {
-                            dx0 = og_wrap(dx0, c); dy0 = og_wrap(dy0, c); dz0 = og_wrap(dz0, c);
-                            dx1 = og_wrap(dx1, c); dy1 = og_wrap(dy1, c); dz1 = og_wrap(dz1, c);
+                            float u0, u1;
+                            upk2(dx, u0, u1); dx = pk2(og_wrap(u0, c), og_wrap(u1, c));
+                            upk2(dy, u0, u1); dy = pk2(og_wrap(u0, c), og_wrap(u1, c));
+                            upk2(dz, u0, u1); dz = pk2(og_wrap(u0, c), og_wrap(u1, c));
                         }
-                        const float r20 = fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0));
-                        const float r21 = fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1));
-                        const float diff0 = x0.x - (GEOM ? c.theta2 * r20 : t.A * r20 * r20);
-                        const float diff1 = x1.x - (GEOM ? c.theta2 * r21 : t.A * r21 * r21);
-                        const uint32_t bit0 = (G == 32 || one) ? (1u << j0) : 0u, bit1 = two ? (1u << j1) : 0u;
-                        const bool cand0 = (Mt & bit0) && !(r20 > x0.z), cand1 = (Mt & bit1) && !(r21 > x1.z);
-                        const bool fopen0 = diff0 > x0.w, fopen1 = diff1 > x1.w;
-                        const bool facc0 = diff0 < -x0.w && r20 > fmaxf(x0.y, hi2m);
-                        const bool facc1 = diff1 < -x1.w && r21 > fmaxf(x1.y, hi2m);
+                        const f32x2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+                        const f32x2 rhs = GEOM ? mul2(r2, A2) : mul2(mul2(r2, A2), r2);   // theta^2 r^2 / (A r^2) r^2
+                        float r20, r21, rh0, rh1;
+                        upk2(r2, r20, r21);
+                        upk2(rhs, rh0, rh1);
+                        const uint32_t bit0 = 1u << (2u * p), bit1 = 2u << (2u * p);
+                        const bool in0 = (__float_as_uint(a3.z) & mybit) != 0u, in1 = (__float_as_uint(a3.w) & mybit) != 0u;
+                        const bool cand0 = in0 && !(r20 > a1.z), cand1 = in1 && !(r21 > a1.w);
+                        const bool fopen0 = rh0 < a2.x, fopen1 = rh1 < a2.y;
+                        const bool facc0 = rh0 > a2.z && r20 > a3.x, facc1 = rh1 > a2.w && r21 > a3.y;
                         or_if(openw, bit0, cand0 && fopen0);
                         or_if(openw, bit1, cand1 && fopen1);
                         or_if(accw, bit0, cand0 && !fopen0 && facc0 && r20 < c.rcut2_hi);
@@ -660,8 +707,8 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                         or_if(sloww, bit0, cand0 && !fopen0 && !facc0);
                         or_if(sloww, bit1, cand1 && !fopen1 && !facc1);
                         if (COUNT) {
-                            if ((Mt & bit0) && !cand0) ++lc.cull;
-                            if ((Mt & bit1) && !cand1) ++lc.cull;
+                            if (in0 && !cand0) ++lc.cull;
+                            if (in1 && !cand1) ++lc.cull;
                             if (cand0 && (fopen0 || facc0)) ++lc.full;
                             if (cand1 && (fopen1 || facc1)) ++lc.full;
                         }
@@ -669,10 +716,9 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     while (sloww) {   // per lane, rare
                         const int j = __ffs(sloww) - 1;
                         sloww &= sloww - 1u;
-                        const float4 s = w.xn_com[j];
-                        const float4 x = w.xn_aux[j];
+                        const float *f = &w.xq[j >> 1][0].x + (j & 1);
                         const float4 cc = w.xn_cel[j];
-                        float dx = s.x - t.x, dy = s.y - t.y, dz = s.z - t.z;
+                        float dx = f[0] - t.x, dy = f[2] - t.y, dz = f[4] - t.z;
                         float ex = cc.x - t.x, ey = cc.y - t.y, ez = cc.z - t.z;
                         if (xwrap) {
                             dx = og_wrap(dx, c); dy = og_wrap(dy, c); dz = og_wrap(dz, c);
@@ -680,19 +726,19 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                         }
                         const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
                         const float rhs = GEOM ? c.theta2 * r2 : t.A * r2 * r2;
-                        const float diff = x.x - rhs;
+                        const bool crit_open = rhs < f[8];
                         const float cmax = fmaxf(fabsf(ex), fmaxf(fabsf(ey), fabsf(ez)));
                         const float lim = 0.6f * cc.w;
                         const float hh2 = fmaxf(hi2, w.xn_hm2[j]);
-                        const bool amb = fabsf(diff) <= x.w || fabsf(cmax - lim) <= OG_BAND * cc.w ||
+                        const bool amb = (!crit_open && !(rhs > f[10])) || fabsf(cmax - lim) <= OG_BAND * cc.w ||
                                          fabsf(r2 - hh2) <= OG_BAND * hh2;
                         bool open, accept;
                         if (amb) {
-                            const int d = slow_decide<GEOM>(a, w.xn_idx[j], t, cnt);
+                            const int d = slow_decide<GEOM>(a, w.xn_u[j], t, cnt);
                             open = d == 1; accept = d == 2;
                             if (COUNT) { if (d == 0) ++lc.cull; else ++lc.full; }
                         } else {
-                            open = diff > 0.0f || cmax < lim || r2 < hh2;
+                            open = crit_open || cmax < lim || r2 < hh2;
                             accept = !open;
                             if (COUNT) ++lc.full;
                         }
@@ -701,13 +747,14 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                         if (accept && r2 < c.rcut2_hi) accw |= bit;
                     }
                     __syncwarp();
-                    myopen = transpose32(openw, lane);   // lane j: the lanes that open the node lane j holds
-                    if (G == 16) myopen = (myopen | (myopen >> 16)) & TMASK;            // -> target mask
-                    if (G == 8) { myopen |= myopen >> 16; myopen = (myopen | (myopen >> 8)) & TMASK; }
-                    if (G == 4) { myopen |= myopen >> 16; myopen |= myopen >> 8; myopen = (myopen | (myopen >> 4)) & TMASK; }
+                    uint32_t ot = transpose32(openw, lane);   // lane j: the lanes that open undecided node j
+                    if (G == 16) ot = (ot | (ot >> 16)) & TMASK;            // -> target mask
+                    if (G == 8) { ot |= ot >> 16; ot = (ot | (ot >> 8)) & TMASK; }
+                    if (G == 4) { ot |= ot >> 16; ot |= ot >> 8; ot = (ot | (ot >> 4)) & TMASK; }
+                    myopen = __shfl_sync(0xffffffffu, ot, rX);   // back to the lane that holds the node
                 }
                 if ((bA | bX) != 0u) {
-                    w.W[head & (GW_NSEG - 1)][lane] = (Mt & bA & myslots) | accw;
+                    w.W[head & (GW_NSEG - 1)][lane] = (MtA & myslots) | accw;
                     if (COUNT && lane == 0) w.seg_flags[head & (GW_NSEG - 1)] = 0u;
                     ++head;
                 }
@@ -721,27 +768,28 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 const uint32_t bn = __ballot_sync(0xffffffffu, push_n);
                 const uint32_t bp = __ballot_sync(0xffffffffu, push_p);
                 const int nn = __popc(bn);
-                if (top + nn > GW_STACK) {  // spill the bottom of the stack to global memory
-                    if (spill_n + GW_SPILL > a.spill_cap) {
+                if ((uint32_t)(top + nn) > a.stack_cap) {  // spill the older half of the stack to global memory
+                    if (spill_n + half > a.spill_cap) {
                         if (lane == 0) atomicOr(a.status, OG_DEV_STACK_OVERFLOW);
                         top = 0;  // give up on this group (result invalid, status latched)
                     } else {
-                        for (uint32_t i = lane; i < (uint32_t)GW_SPILL; i += 32) {
+                        for (uint32_t i = lane; i < half; i += 32) {
                             sp_start[spill_n + i] = w.st_start[i];
                             sp_cnt[spill_n + i] = w.st_cnt[i];
                             sp_mask[spill_n + i] = w.st_mask[i];
                         }
                         __syncwarp();
-                        const uint32_t rest = (uint32_t)top - GW_SPILL;
+                        const uint32_t rest = (uint32_t)top - half;
                         for (uint32_t i0 = 0; i0 < rest; i0 += 32) {
                             const uint32_t i = i0 + lane;
                             uint32_t s0 = 0, s1 = 0, s2 = 0;
-                            if (i < rest) { s0 = w.st_start[i + GW_SPILL]; s1 = w.st_cnt[i + GW_SPILL]; s2 = w.st_mask[i + GW_SPILL]; }
+                            if (i < rest) { s0 = w.st_start[i + half]; s1 = w.st_cnt[i + half]; s2 = w.st_mask[i + half]; }
                             __syncwarp();
                             if (i < rest) { w.st_start[i] = s0; w.st_cnt[i] = s1; w.st_mask[i] = s2; }
                         }
-                        spill_n += GW_SPILL;
-                        top -= GW_SPILL;
+                        spill_n += half;
+                        top -= (int)half;
+                        if (COUNT && lane == 0) atomicAdd(&a.counters[OGC_SPILLS], 1ull);
                         __syncwarp();
                     }
                 }
@@ -809,6 +857,14 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                 __syncwarp();
             }
         }
+        Accum acc;
+        {
+            float a, b;
+            upk2(acc2.ax, a, b); acc.ax = a + b;
+            upk2(acc2.ay, a, b); acc.ay = a + b;
+            upk2(acc2.az, a, b); acc.az = a + b;
+            upk2(acc2.pot, a, b); acc.pot = -(a + b);
+        }
         if (G < 32) {   // add the K partial sums of every target
 #pragma unroll
             for (int o = G; o < 32; o <<= 1) {
@@ -821,15 +877,6 @@ k_walk_group(const __grid_constant__ WalkArgs a)
             a.acc_out[3 * (size_t)out + 1] = acc.ay;
             a.acc_out[3 * (size_t)out + 2] = acc.az;
             if (POT) a.pot_out[out] = acc.pot;
-        }
-        if (COUNT && lane == 0) {
-            const float e = fmaxf(g.ghx, fmaxf(g.ghy, g.ghz)) / c.rcut;
-            const int b = e < 0.025f ? 0 : e < 0.05f ? 1 : e < 0.1f ? 2 : e < 0.2f ? 3 : e < 0.4f ? 4 : 5;
-            atomicAdd(&a.counters[OGC_DIAG0 + b], 1ull);
-            atomicAdd(&a.counters[OGC_DIAG0 + 6 + b], (unsigned long long)(clock64() - dg_t0));
-            atomicAdd(&a.counters[OGC_DIAG0 + 12 + b], (unsigned long long)dg_gen);
-            atomicAdd(&a.counters[OGC_DIAG0 + 18 + b], (unsigned long long)head);
-            atomicAdd(&a.counters[OGC_DIAG0 + 24 + b], (unsigned long long)(lc.ain + lc.pin));
         }
         if (COUNT) {
             const uint32_t v[6] = {lc.full, lc.cull, lc.ain, lc.pin, lc.psoft, lc.pout};
@@ -846,11 +893,6 @@ k_walk_group(const __grid_constant__ WalkArgs a)
 template <bool GEOM, bool POT, bool COUNT>
 cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
 {
-    if (t->prm.walk_variant == OG_WALK_SIMPLE) {
-        const unsigned grid = (a.n_active + 127) / 128;
-        k_walk_simple<GEOM, POT, COUNT><<<grid, 128, 0, st>>>(a);
-        return cudaGetLastError();
-    }
     // Targets per warp: 32 when the active targets are dense in Morton order; 8 (4 lanes per target) for a
     // sparse active subset, whose 32 consecutive targets would span many cells (zoom: 52 -> 31 ms).  For the
     // spread-out groups of a DENSE target set (uniform background of nfw256) 8 per warp is slower (measured).
@@ -865,7 +907,7 @@ cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, GW_THREADS, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
-    if (per_sm * GW_WARPS > 32) per_sm = 32 / GW_WARPS;   // spill slabs are sized for <= 32 warps per SM
+    if (per_sm > OG_GW_MINBLOCKS) per_sm = OG_GW_MINBLOCKS;   // the spill slabs are sized for this many blocks per SM
     const unsigned grid = (unsigned)(per_sm * t->sm_count);
     kern<<<grid, GW_THREADS, smem, st>>>(a);
     return cudaGetLastError();
@@ -873,11 +915,14 @@ cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
 
 }  // namespace
 
-static constexpr uint32_t SPILL_CAP = 3072;  // entries per warp (x 12 B)
-
-size_t ogk_walk_spill_bytes(int sm_count)
+uint32_t ogk_walk_spill_entries(const og_params *p)
 {
-    return (size_t)sm_count * 32 * 3 * SPILL_CAP * sizeof(uint32_t);   // up to 32 resident warps per SM
+    return p->walk_spill_entries ? p->walk_spill_entries : 3072u;   // ranges per warp (x 12 B)
+}
+
+size_t ogk_walk_spill_bytes(int sm_count, uint32_t spill_entries)
+{
+    return (size_t)sm_count * OG_GW_MINBLOCKS * GW_WARPS * 3 * spill_entries * sizeof(uint32_t);
 }
 
 cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out, uint64_t n_active,
@@ -893,7 +938,8 @@ cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t 
     a.status = t->d_status;
     a.counters = t->d_counters;
     a.spill = reinterpret_cast<uint32_t *>(t->walk_spill);
-    a.spill_cap = SPILL_CAP;
+    a.spill_cap = t->walk_spill_cap;
+    a.stack_cap = t->prm.walk_stack_entries ? min(t->prm.walk_stack_entries, (uint32_t)GW_STACK) : (uint32_t)GW_STACK;
     const og_params &p = t->prm;
     WalkConst &c = a.c;
     c.dL = (double)t->box;

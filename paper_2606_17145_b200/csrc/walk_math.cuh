@@ -50,6 +50,19 @@ __device__ __forceinline__ double og_wrap64(double d, double L) { return d - L *
 // Split factors (R18) in registers: E(w) = erfc(w) = exp(-w^2) P(w), T(w) = E(w) + (2 / sqrt(pi)) w exp(-w^2),
 // w = r / (2 r_s).  P = degree-10 polynomial, weighted-minimax fit of erfcx on [0, OG_WMAX] (weight exp(-w^2));
 // exp(-w^2) = ex2.approx(r^2 k_e).  Max abs error of T and E in fp32 Horner: 1.8e-7 (budget 1e-6).
+// Coefficients of P (degree 10, highest first: OG_SP10 .. OG_SP0), shared by og_split and og_split2.
+#define OG_SP10 1.651949088e-04f
+#define OG_SP9 -2.225770333e-03f
+#define OG_SP8 1.362162625e-02f
+#define OG_SP7 -5.118135848e-02f
+#define OG_SP6 1.361394758e-01f
+#define OG_SP5 -2.828231287e-01f
+#define OG_SP4 4.931623193e-01f
+#define OG_SP3 -7.507289497e-01f
+#define OG_SP2 9.998254850e-01f
+#define OG_SP1 -1.128371385e+00f
+#define OG_SP0 9.999999427e-01f
+#define OG_TWO_OVER_SQRTPI 1.1283791670955126f
 __device__ __forceinline__ float og_ex2(float x)
 {
     float y;
@@ -69,19 +82,88 @@ __device__ __forceinline__ void og_split(float r, float r2, const WalkConst &c, 
 {
     const float w = r * c.k_w;
     const float ex = og_ex2(r2 * c.k_e);
-    float p = 1.651949088e-04f;
-    p = fmaf(p, w, -2.225770333e-03f);
-    p = fmaf(p, w, 1.362162625e-02f);
-    p = fmaf(p, w, -5.118135848e-02f);
-    p = fmaf(p, w, 1.361394758e-01f);
-    p = fmaf(p, w, -2.828231287e-01f);
-    p = fmaf(p, w, 4.931623193e-01f);
-    p = fmaf(p, w, -7.507289497e-01f);
-    p = fmaf(p, w, 9.998254850e-01f);
-    p = fmaf(p, w, -1.128371385e+00f);
-    p = fmaf(p, w, 9.999999427e-01f);
+    float p = OG_SP10;
+    p = fmaf(p, w, OG_SP9);
+    p = fmaf(p, w, OG_SP8);
+    p = fmaf(p, w, OG_SP7);
+    p = fmaf(p, w, OG_SP6);
+    p = fmaf(p, w, OG_SP5);
+    p = fmaf(p, w, OG_SP4);
+    p = fmaf(p, w, OG_SP3);
+    p = fmaf(p, w, OG_SP2);
+    p = fmaf(p, w, OG_SP1);
+    p = fmaf(p, w, OG_SP0);
     E = p * ex;
-    T = fmaf(1.1283791670955126f * w, ex, E);
+    T = fmaf(OG_TWO_OVER_SQRTPI * w, ex, E);
+}
+
+// ---- packed fp32 pairs (sm_100: fma/mul/add/sub.rn.f32x2 -> FFMA2 / FMUL2 / FADD2) ---------------
+// One instruction, two independent IEEE fp32 operations on a 64-bit register pair: the two source chains
+// of the consume loop and the two nodes of an undecided-node test are pairs of identical operations, so
+// packing them halves their issue slots (the walk is issue-bound).  Each half rounds
+// exactly like the scalar instruction.
+typedef unsigned long long f32x2;
+
+__device__ __forceinline__ f32x2 pk2(float a, float b)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ void upk2(f32x2 v, float &a, float &b)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 bc2(float a) { return pk2(a, a); }
+
+// og_split for two sources at once, same coefficients.  The polynomial is evaluated as even and odd part
+// in w^2 (two independent Horner chains, depth 7 instead of 10: the walk is latency-bound at its occupancy),
+// P(w) = Pe(w^2) + w Po(w^2); tests/test_split_poly.py evaluates this order in fp32 against the R18 budget.
+__device__ __forceinline__ void og_split2(f32x2 r, f32x2 r2, const WalkConst &c, f32x2 &T, f32x2 &E)
+{
+    const f32x2 w = mul2(r, bc2(c.k_w));
+    const f32x2 a = mul2(r2, bc2(c.k_e));
+    float a0, a1;
+    upk2(a, a0, a1);
+    const f32x2 ex = pk2(og_ex2(a0), og_ex2(a1));
+    const f32x2 w2 = mul2(w, w);
+    f32x2 pe = bc2(OG_SP10), po = bc2(OG_SP9);
+    pe = fma2(pe, w2, bc2(OG_SP8));
+    po = fma2(po, w2, bc2(OG_SP7));
+    pe = fma2(pe, w2, bc2(OG_SP6));
+    po = fma2(po, w2, bc2(OG_SP5));
+    pe = fma2(pe, w2, bc2(OG_SP4));
+    po = fma2(po, w2, bc2(OG_SP3));
+    pe = fma2(pe, w2, bc2(OG_SP2));
+    po = fma2(po, w2, bc2(OG_SP1));
+    pe = fma2(pe, w2, bc2(OG_SP0));
+    const f32x2 p = fma2(po, w, pe);
+    E = mul2(p, ex);
+    T = fma2(mul2(w, bc2(OG_TWO_OVER_SQRTPI)), ex, E);
 }
 
 // ---- cutoff decision r < r_cut (R17, strict) ------------------------------------------------

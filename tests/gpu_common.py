@@ -14,11 +14,13 @@ def oracle_params(w, leaf_max=8, alpha=None, theta=None):
                               theta=w.theta if theta is None else theta, leaf_max=leaf_max)
 
 
-def gpu_params(w, leaf_max=8, flags=0, walk_variant=0, alpha=None, theta=None, max_nodes=0):
+def gpu_params(w, leaf_max=8, flags=0, alpha=None, theta=None, max_nodes=0, walk_stack_entries=0,
+               walk_spill_entries=0):
     from paper_2606_17145_b200 import binding as B
     return B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha if alpha is None else alpha,
                          theta=w.theta if theta is None else theta, leaf_max=leaf_max, max_nodes=max_nodes,
-                         flags=B.OG_PERIODIC | flags, walk_variant=walk_variant)
+                         flags=B.OG_PERIODIC | flags, walk_stack_entries=walk_stack_entries,
+                         walk_spill_entries=walk_spill_entries)
 
 
 def to_dev(w):

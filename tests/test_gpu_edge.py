@@ -218,3 +218,82 @@ def test_mixed_softening_species(B):
     check_acc(a3, ao3, what="species sparse")
     ep = rel_err_scalar(p3, po3)
     assert np.percentile(ep, 99) <= 1e-4 and ep.max() <= 1e-2
+
+
+# ---- traversal stack: spill / reload path and the capacity latch (og_params.walk_stack_entries / walk_spill_entries) ----
+def _spill_case(B, stack_entries, spill_entries):
+    import torch
+    w = W.make("nfw256", small=True)
+    prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=1,
+                        max_nodes=3 * w.n, flags=B.OG_PERIODIC | B.OG_COUNT, walk_stack_entries=stack_entries,
+                        walk_spill_entries=spill_entries)
+    pos, mass, eps = (torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps))
+    tree = B.og_tree_build(pos, mass, eps, w.L, prm)
+    a, p = B.og_shortrange_accel(tree, None, None)
+    st = B.og_tree_stats(tree)
+    status = B.og_tree_status(tree)
+    B.og_tree_free(tree)
+    return w, a.cpu().numpy(), p.cpu().numpy(), st, status
+
+
+def test_stack_spill_and_reload_keep_parity(B):
+    """A 64-entry shared-memory stack on a leaf_max = 1 tree forces the warps to move ranges to their global slabs
+    and back (stack_spills > 0); the walk still equals the oracle's, and visits exactly the same nodes as the run
+    with the default stack (equal counters)."""
+    w, a, p, st, status = _spill_case(B, 64, 0)
+    assert status == B.OG_OK, B.og_last_error()
+    assert st["stack_spills"] > 0, st
+    w2, a2, p2, st2, status2 = _spill_case(B, 0, 0)
+    assert status2 == B.OG_OK and st2["stack_spills"] == 0
+    for k in ("V_full", "V_cull", "A_in", "P_in", "P_soft", "P_out"):
+        assert st[k] == st2[k], (k, st[k], st2[k])
+    ot = oracle.build_tree(w.pos, w.mass, w.eps, oracle.make_params(w.L, w.r_s, G=w.G, alpha=w.alpha, theta=w.theta,
+                                                                     leaf_max=1))
+    ao, po, _ = oracle.walk(ot, None, None, want_counters=False)
+    check_acc(a, ao, what="spilled stack")
+    ep = rel_err_scalar(p, po)
+    assert np.percentile(ep, 99) <= 1e-4 and ep.max() <= 1e-2
+
+
+def test_stack_overflow_is_latched(B):
+    """A slab too small for the first spill (16 < 64 / 2 ranges): OG_ERR_STACK_OVERFLOW is latched, nothing faults."""
+    _, a, p, st, status = _spill_case(B, 64, 16)
+    assert status == B.OG_ERR_STACK_OVERFLOW
+    assert np.all(np.isfinite(a))
+
+
+def test_bad_stack_knobs_are_rejected(B):
+    import torch
+    w = W.make("uniform32", small=True)
+    pos, mass, eps = (torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps))
+    for bad in (32, 65, 512):
+        with pytest.raises(B.OgError):
+            B.og_tree_build(pos, mass, eps, w.L, B.make_params(w.r_s, walk_stack_entries=bad))
+
+
+# ---- streams (og.h "Streams and a tree") ---------------------------------------------------------------
+def test_walks_on_other_streams_are_ordered_after_build_and_each_other(B):
+    """Build on one stream, walk at once on two others without any host synchronisation in between: the library
+    orders the walks after the build and after each other (they share the tree's scratch state), so the results
+    are bit-identical to the single-stream run."""
+    import torch
+    w = W.make("nfw256", small=True)
+    pos, mass, eps = (torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps))
+    prm = B.make_params(w.r_s, G=w.G, alpha=w.alpha, theta=w.theta)
+    tree = B.og_tree_build(pos, mass, eps, w.L, prm)
+    a_ref, p_ref = B.og_shortrange_accel(tree, None, None)
+    a_old = torch.linalg.vector_norm(a_ref, dim=1).contiguous()
+    a_ref2, p_ref2 = B.og_shortrange_accel(tree, None, a_old)
+    torch.cuda.synchronize()
+    B.og_tree_free(tree)
+    s0, s1, s2 = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    for rep in range(3):
+        torch.cuda.synchronize()
+        tree = B.og_tree_build(pos, mass, eps, w.L, prm, stream=s0)
+        a1, p1 = B.og_shortrange_accel(tree, None, None, stream=s1)
+        a2, p2 = B.og_shortrange_accel(tree, None, a_old, stream=s2)
+        B.og_tree_free(tree, stream=s0)          # ordered after the last walk by the library
+        torch.cuda.synchronize()
+        assert torch.equal(a1, a_ref) and torch.equal(p1, p_ref)
+        assert torch.equal(a2, a_ref2) and torch.equal(p2, p_ref2)
+    B.og_trim()

@@ -118,11 +118,11 @@ def test_tree_bit_exact(B, name, leaf_max):
 
 
 # ---- a6..a7: walk ---------------------------------------------------------------------------
-def _walk_case(B, name, variant, leaf_max=8):
+def _walk_case(B, name, leaf_max=8):
     import torch
     w, t = _case(name, leaf_max)
     pos, mass, eps = to_dev(w)
-    tree = B.og_tree_build(pos, mass, eps, w.L, gpu_params(w, leaf_max, flags=B.OG_COUNT, walk_variant=variant))
+    tree = B.og_tree_build(pos, mass, eps, w.L, gpu_params(w, leaf_max, flags=B.OG_COUNT))
     act = None if w.active_idx is None else torch.from_numpy(w.active_idx.view(np.int32)).cuda()
     # pass 1: geometric criterion (theta = 0.5), parity-checked on its own (R23)
     a1, p1 = B.og_shortrange_accel(tree, act, None)
@@ -150,12 +150,7 @@ def _walk_case(B, name, variant, leaf_max=8):
 
 @pytest.mark.parametrize("name", SMALL)
 def test_walk_group_matches_oracle(B, name):
-    _walk_case(B, name, 0)
-
-
-@pytest.mark.parametrize("name", ["uniform32", "nfw256", "zoom"])
-def test_walk_simple_matches_oracle(B, name):
-    _walk_case(B, name, 1)
+    _walk_case(B, name)
 
 
 @pytest.mark.parametrize("leaf_max", [1, 32])

@@ -32,11 +32,19 @@ def test_header_symbols_exported(B):
     assert set(B.EXPORTS) == set(names)
 
 
+def test_only_the_documented_calls_are_exported(B):
+    """nm -D: the og_* symbols of libogtree.so are exactly the calls og.h declares (no bench / debug helpers)."""
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", B.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    exported = sorted(set(re.findall(r"\b(og_[a-z0-9_]+)\b", out)))
+    assert exported == _declared_symbols(), exported
+
+
 def test_params_struct_matches_header(B):
     p = B.make_params(0.01)
     assert p.struct_size == C.sizeof(B.og_params)
-    # uint32 x2, float x5, uint32 x3, pointer, size_t
-    assert C.sizeof(B.og_params) == 40 + 8 + 8
+    # uint32 x2, float x5, uint32 x4, (4 bytes padding), pointer, size_t
+    assert C.sizeof(B.og_params) == 48 + 8 + 8
 
 
 def test_workspace_bytes_is_host_only(B):
