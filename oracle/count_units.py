@@ -50,7 +50,9 @@ def count(name: str, sample: int, small: bool, seed: int = 12345) -> dict:
         "F_alg_per_target": float(F_alg.mean()), "F_int_per_target": float(F_int.mean()),
         "F_alg_per_target_nopot": float(F_alg_np.mean()), "F_int_per_target_nopot": float(F_int_np.mean()),
         "interactions_per_target": float(mean[2] + mean[4]),
-        "compulsory_hbm_bytes": int(t.n_nodes * 72 + w.n * 20 + w.n_active * 40),
+        # every packed 48-byte walk record and every sorted particle (float4 + h) once; per active target: index 4,
+        # a_old 4, gathered position 16, acc 12, pot 4
+        "compulsory_hbm_bytes": int(t.n_nodes * 48 + w.n * 20 + w.n_active * 40),
         "weights": oracle.FLOP_WEIGHTS, "weights_nopot": oracle.FLOP_WEIGHTS_NOPOT,
         "oracle_build_s": t_build, "oracle_two_pass_walk_s": t_walk2, "oracle_threads": oracle.num_threads(),
     }
