@@ -202,6 +202,30 @@ int og_shortrange_accel_host(const float *pos, const float *mass, const float *s
                              uint64_t n_active, const float *a_old, float *acc_out,
                              float *pot_out, og_stream stream);
 
+/* ---- row f1: the PM long-range part of the TreePM force ------------------------------- */
+
+/*
+ * PAPER.md:124 keeps the long-range PM force on the CPU (FFTW); here it runs on the device.  Together with
+ * og_shortrange_accel (same r_s, same G) it gives the full periodic Newtonian force within the TreePM error.
+ * Steps (readings R31..R34; Gadget-2 lineage): CIC assignment of the masses to
+ * ng^3 grid points -> DFT (cuFFT, the one library step) -> phi_k = -4 pi G / (V k^2) exp(-k^2 r_s^2) M_k / W(k)^2
+ * (W = CIC window, divided out twice; phi_0 = 0) -> inverse DFT -> 4-point finite-difference gradient ->
+ * CIC interpolation of acceleration and potential to the targets.  fp32 throughout.
+ *
+ * og_pm_create: plans and grids for an ng^3 mesh (ng even, 8..2048; Gadget's choice is r_s = 1.25 box / ng);
+ *   device memory ~ 28 ng^3 bytes, owned by the handle.  Synchronises `stream` once.  NULL on failure.
+ * og_pm_longrange: all pointers DEVICE.  pos f32 [n][3] in [0, box), mass f32 [n] (all n particles are sources);
+ *   active_idx u32 [n_active] original indices of the targets, or NULL -> all n in identity order
+ *   (n_active == n); acc_out f32 [n_active][3], pot_out f32 [n_active] or NULL, overwritten.  Enqueues on `stream`.
+ *   The mass assignment uses floating-point atomics: results are reproducible to fp32 rounding, not bit for bit.
+ * og_pm_free: synchronises `stream`, releases plans and grids.  NULL is ignored.
+ */
+typedef struct og_pm og_pm;
+og_pm *og_pm_create(uint32_t ng, float box, float r_s, float G, og_stream stream);
+int og_pm_longrange(og_pm *pm, const float *pos, const float *mass, uint64_t n, const uint32_t *active_idx,
+                    uint64_t n_active, float *acc_out, float *pot_out, og_stream stream);
+void og_pm_free(og_pm *pm, og_stream stream);
+
 /* Returns the device memory that freed trees / finished calls left cached in the library's
  * stream-ordered pool of the current device to the driver (the pool keeps arenas for reuse by
  * the next og_tree_build; a host code that needs the memory for something else calls this).

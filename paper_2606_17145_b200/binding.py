@@ -105,6 +105,12 @@ def _load():
                                              vp, vp]
     lib.og_trim.restype = C.c_int
     lib.og_trim.argtypes = []
+    lib.og_pm_create.restype = vp
+    lib.og_pm_create.argtypes = [C.c_uint32, C.c_float, C.c_float, C.c_float, vp]
+    lib.og_pm_longrange.restype = C.c_int
+    lib.og_pm_longrange.argtypes = [vp, vp, vp, u64, u32p, u64, vp, vp, vp]
+    lib.og_pm_free.restype = None
+    lib.og_pm_free.argtypes = [vp, vp]
     return lib
 
 
@@ -112,7 +118,8 @@ _lib = _load()
 
 EXPORTS = ("og_tree_workspace_bytes", "og_tree_build", "og_shortrange_accel", "og_tree_get", "og_tree_status",
            "og_tree_stats", "og_tree_free", "og_last_error", "og_morton_keys", "og_radix_sort_scratch_bytes",
-           "og_radix_sort_pairs", "og_shortrange_accel_host", "og_trim")
+           "og_radix_sort_pairs", "og_shortrange_accel_host", "og_trim", "og_pm_create", "og_pm_longrange",
+           "og_pm_free")
 
 
 def _err() -> str:
@@ -294,3 +301,45 @@ def og_shortrange_accel_host(pos, mass, soft, box: float, params: og_params, act
 def og_trim():
     """Returns the memory cached in the library's stream-ordered pool to the driver."""
     _check(_lib.og_trim())
+
+
+# ---- row f1: PM long-range force -------------------------------------------------------------------------
+class Pm:
+    def __init__(self, handle: int, ng: int, box: float):
+        self.handle, self.ng, self.box = handle, ng, box
+
+    def __del__(self):
+        try:
+            og_pm_free(self)
+        except Exception:
+            pass
+
+
+def og_pm_create(ng: int, box: float, r_s: float, G: float = 1.0, stream=None) -> Pm:
+    h = _lib.og_pm_create(int(ng), float(box), float(r_s), float(G), _stream(stream))
+    if not h:
+        raise OgError(OG_ERR_INVALID_ARG, _err())
+    return Pm(h, int(ng), float(box))
+
+
+def og_pm_longrange(pm: Pm, pos: torch.Tensor, mass: torch.Tensor, active_idx: torch.Tensor | None = None,
+                    want_pot: bool = True, stream=None):
+    """-> (acc [na][3], pot [na] | None): long-range acceleration and potential at the targets."""
+    n = int(pos.shape[0])
+    na = n if active_idx is None else int(active_idx.shape[0])
+    acc = torch.empty((na, 3), dtype=torch.float32, device=pos.device)
+    pot = torch.empty((na,), dtype=torch.float32, device=pos.device) if want_pot else None
+    ai = None
+    if active_idx is not None:
+        if active_idx.dtype not in (torch.int32, torch.uint32) or not (active_idx.is_cuda and active_idx.is_contiguous()):
+            raise TypeError("active_idx must be a contiguous int32 / uint32 CUDA tensor")
+        ai = active_idx.data_ptr()
+    _check(_lib.og_pm_longrange(pm.handle, _dev(pos, torch.float32, "pos"), _dev(mass, torch.float32, "mass"), n, ai, na,
+                                acc.data_ptr(), None if pot is None else pot.data_ptr(), _stream(stream)))
+    return acc, pot
+
+
+def og_pm_free(pm: Pm, stream=None):
+    if pm.handle:
+        h, pm.handle = pm.handle, 0
+        _lib.og_pm_free(h, _stream(stream) if torch.cuda.is_available() else None)

@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libogtree.so")
 PROBE_LIB = os.path.join(HERE, "libogprobe.so")
-SOURCES = ["api.cu", "keys.cu", "radix_sort.cu", "octree.cu", "walk.cu"]
+SOURCES = ["api.cu", "keys.cu", "radix_sort.cu", "octree.cu", "walk.cu", "pm.cu"]
 PROBE_SOURCES = ["probe.cu"]
 HEADERS = ["og_internal.cuh", "walk_math.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
@@ -66,7 +66,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if failed:
         raise RuntimeError("nvcc failed (see output above)")
     n = len(SOURCES)
-    subprocess.run([_nvcc(), "-shared", "-o", LIB, *objs[:n]], check=True)  # static cudart (nvcc default)
+    # static cudart (nvcc default); cuFFT (the DFT of the PM step) from the toolkit's shared library
+    subprocess.run([_nvcc(), "-shared", "-o", LIB, *objs[:n], "-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"],
+                   check=True)
     subprocess.run([_nvcc(), "-shared", "-o", PROBE_LIB, *objs[n:]], check=True)
     return LIB
 
