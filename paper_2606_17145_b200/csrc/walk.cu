@@ -89,8 +89,8 @@ __device__ __forceinline__ Target load_target(const WalkArgs &a, uint32_t k, uin
 #ifndef OG_GW_STACK
 #define OG_GW_STACK 256
 #endif
-#ifndef OG_CONSUME_PIPELINED
-#define OG_CONSUME_PIPELINED 0
+#ifndef OG_CONSUME_FOUR
+#define OG_CONSUME_FOUR 1   // two takes (4 sources) per consume iteration: nfw256 49.2 -> 48.2 ms
 #endif
 constexpr int GW_WARPS = OG_GW_WARPS;           // warps per block
 constexpr int GW_THREADS = GW_WARPS * 32;
@@ -365,9 +365,9 @@ __device__ __forceinline__ void take_two(WarpSmem &w, LanePos &lp, const uint32_
 // pairs (FFMA2 / FMUL2, walk_math.cuh).  Newtonian monopole x split factor (R21); a source that is within
 // OG_BAND of r_cut or closer than the largest softening length of the whole particle set goes to pair_exact.
 template <bool POT, bool COUNT, bool WRAP, bool HLOOK>
-__device__ __forceinline__ void eval_two(WarpSmem &w, const float4 q0, const float4 q1, const uint32_t e0, const uint32_t e1,
-                                         const Target &t, const float hmax2g, const WalkConst &c, Accum2 &acc,
-                                         unsigned long long *cnt, LaneCount &lc)
+__device__ __forceinline__ uint32_t eval_two_fast(WarpSmem &w, const float4 q0, const float4 q1, const uint32_t e0,
+                                                  const uint32_t e1, const Target &t, const float hmax2g,
+                                                  const WalkConst &c, Accum2 &acc)
 {
     const bool v0 = e0 != GW_DUMMY, v1 = e1 != GW_DUMMY;
     float dx0 = q0.x - t.x, dy0 = q0.y - t.y, dz0 = q0.z - t.z;
@@ -380,27 +380,73 @@ __device__ __forceinline__ void eval_two(WarpSmem &w, const float4 q0, const flo
     const f32x2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
     float r20, r21;
     upk2(r2, r20, r21);
-    // fast: strictly inside the cutoff band and not softened: anything closer than the largest h of the
-    // whole particle set (h_max of the root) takes the exact path.  HLOOK (the 8-targets-per-warp kernel,
-    // used for sparse active subsets, where a multi-species zoom has h comparable to r_cut): the source's
-    // own h is looked up below that bound (nodes carry h = 0: R16 keeps accepted nodes outside the
-    // target's own h).
-    bool fast0, fast1;
     if (HLOOK) {
-        bool soft0 = r20 < hmax2g, soft1 = r21 < hmax2g;
+        // The 8-targets-per-warp kernel (sparse active subsets; a multi-species zoom has h comparable to r_cut and
+        // most of its pairs softened: config 4 has 578 of 860 pairs per target inside h): the source's own h is
+        // looked up below the largest h of the particle set (nodes carry h = 0: R16 keeps accepted nodes outside
+        // the target's own h), and the spline-softened kernel (C5) is evaluated HERE, both polynomial pieces as
+        // packed pairs and selected by u = r / h; g and p are continuous at u = 1/2 and u = 1, so only the cutoff
+        // band (and r = 0) needs the exact path.
+        const bool near0 = r20 < hmax2g, near1 = r21 < hmax2g;
         float hj0 = 0.0f, hj1 = 0.0f;
-        if ((!WRAP || v0) && soft0) hj0 = w.ring_h[e0];
-        if ((!WRAP || v1) && soft1) hj1 = w.ring_h[e1];
+        if ((!WRAP || v0) && near0) hj0 = w.ring_h[e0];
+        if ((!WRAP || v1) && near1) hj1 = w.ring_h[e1];
         const float hh0 = fmaxf(t.h, hj0), hh1 = fmaxf(t.h, hj1);
-        soft0 = soft0 && r20 < hh0 * hh0 * (1.0f + OG_BAND);
-        soft1 = soft1 && r21 < hh1 * hh1 * (1.0f + OG_BAND);
-        fast0 = (!WRAP || v0) && r20 < c.rcut2_lo && !soft0;
-        fast1 = (!WRAP || v1) && r21 < c.rcut2_lo && !soft1;
-    } else {
-        // (the wrapped distance of the dummy slot is arbitrary: WRAP keeps the validity predicates)
-        fast0 = (!WRAP || v0) && r20 < c.rcut2_lo && r20 >= hmax2g;
-        fast1 = (!WRAP || v1) && r21 < c.rcut2_lo && r21 >= hmax2g;
+        const bool fast0 = (!WRAP || v0) && r20 < c.rcut2_lo && r20 > 1.0e-30f;
+        const bool fast1 = (!WRAP || v1) && r21 < c.rcut2_lo && r21 > 1.0e-30f;
+        const bool soft0 = fast0 && near0 && r20 < hh0 * hh0, soft1 = fast1 && near1 && r21 < hh1 * hh1;
+        const bool slow0 = (!WRAP || v0) && !fast0 && r20 < c.rcut2_hi;
+        const bool slow1 = (!WRAP || v1) && !fast1 && r21 < c.rcut2_hi;
+        const f32x2 ri = pk2(fast0 ? og_rsqrt(r20) : 0.0f, fast1 ? og_rsqrt(r21) : 0.0f);
+        const f32x2 r = mul2(r2, ri);
+        f32x2 T, E;
+        og_split2(r, r2, c, T, E);
+        const f32x2 gm = pk2(fast0 ? q0.w : 0.0f, fast1 ? q1.w : 0.0f);
+        f32x2 gfac = mul2(mul2(ri, ri), ri), pfac = ri;          // Newtonian: 1 / r^3, 1 / r (pot holds +sum)
+        if (__any_sync(0xffffffffu, soft0 || soft1)) {
+            const f32x2 hh = pk2(hh0, hh1);
+            const f32x2 hinv = pk2(soft0 ? __frcp_rn(hh0) : 0.0f, soft1 ? __frcp_rn(hh1) : 0.0f);
+            const f32x2 u = mul2(r, hinv), u2 = mul2(u, u);
+            const f32x2 ui = mul2(hh, ri), ui3 = mul2(mul2(ui, ui), ui);            // 1 / u, 1 / u^3
+            // u < 1/2:  g h^3 = 32/3 + u^2 (32 u - 192/5),  p h = -14/5 + u^2 (16/3 + u^2 (32/5 u - 48/5))
+            f32x2 gi = fma2(u, bc2(32.0f), bc2(-38.4f));
+            gi = fma2(u2, gi, bc2(10.666666666666666f));
+            f32x2 pi = fma2(u, bc2(6.4f), bc2(-9.6f));
+            pi = fma2(u2, pi, bc2(5.333333333333333f));
+            pi = fma2(u2, pi, bc2(-2.8f));
+            // 1/2 <= u < 1:  g h^3 = 64/3 - 48 u + 192/5 u^2 - 32/3 u^3 - 1 / (15 u^3),
+            //                p h = -16/5 + 1 / (15 u) + u^2 (32/3 + u (-16 + u (48/5 - 32/15 u)))
+            f32x2 go = fma2(u, bc2(-10.666666666666666f), bc2(38.4f));
+            go = fma2(u, go, bc2(-48.0f));
+            go = fma2(u, go, bc2(21.333333333333332f));
+            go = fma2(ui3, bc2(-0.06666666666666667f), go);
+            f32x2 po = fma2(u, bc2(-2.1333333333333333f), bc2(9.6f));
+            po = fma2(u, po, bc2(-16.0f));
+            po = fma2(u, po, bc2(10.666666666666666f));
+            po = fma2(u2, po, bc2(-3.2f));
+            po = fma2(ui, bc2(0.06666666666666667f), po);
+            float u0, u1, gi0, gi1, go0, go1, pi0, pi1, po0, po1;
+            upk2(u, u0, u1); upk2(gi, gi0, gi1); upk2(go, go0, go1); upk2(pi, pi0, pi1); upk2(po, po0, po1);
+            const f32x2 gsel = pk2(u0 < 0.5f ? gi0 : go0, u1 < 0.5f ? gi1 : go1);
+            const f32x2 psel = pk2(u0 < 0.5f ? pi0 : po0, u1 < 0.5f ? pi1 : po1);
+            const f32x2 gs = mul2(mul2(mul2(hinv, hinv), hinv), gsel);
+            const f32x2 ps = mul2(mul2(hinv, bc2(-1.0f)), psel);                    // -p > 0
+            float gn0, gn1, pn0, pn1, gs0, gs1, ps0, ps1;
+            upk2(gfac, gn0, gn1); upk2(pfac, pn0, pn1); upk2(gs, gs0, gs1); upk2(ps, ps0, ps1);
+            gfac = pk2(soft0 ? gs0 : gn0, soft1 ? gs1 : gn1);
+            pfac = pk2(soft0 ? ps0 : pn0, soft1 ? ps1 : pn1);
+        }
+        const f32x2 f = mul2(mul2(gm, T), gfac);
+        acc.ax = fma2(f, dx, acc.ax); acc.ay = fma2(f, dy, acc.ay); acc.az = fma2(f, dz, acc.az);
+        if (POT) acc.pot = fma2(mul2(gm, E), pfac, acc.pot);
+        return (slow0 ? 1u : 0u) | (slow1 ? 2u : 0u) |
+               (COUNT ? ((fast0 ? 4u : 0u) | (fast1 ? 8u : 0u) | (soft0 ? 16u : 0u) | (soft1 ? 32u : 0u)) : 0u);
     }
+    // G = 32: fast = strictly inside the cutoff band and not softened: anything closer than the largest h of the
+    // whole particle set (h_max of the root) takes the exact path.
+    // (the wrapped distance of the dummy slot is arbitrary: WRAP keeps the validity predicates)
+    const bool fast0 = (!WRAP || v0) && r20 < c.rcut2_lo && r20 >= hmax2g;
+    const bool fast1 = (!WRAP || v1) && r21 < c.rcut2_lo && r21 >= hmax2g;
     const bool slow0 = (!WRAP || v0) && !fast0 && r20 < c.rcut2_hi;
     const bool slow1 = (!WRAP || v1) && !fast1 && r21 < c.rcut2_hi;
     {
@@ -417,23 +463,43 @@ __device__ __forceinline__ void eval_two(WarpSmem &w, const float4 q0, const flo
         acc.ax = fma2(f, dx, acc.ax); acc.ay = fma2(f, dy, acc.ay); acc.az = fma2(f, dz, acc.az);
         if (POT) acc.pot = fma2(gr, E, acc.pot);
     }
-    int k0 = fast0 ? 1 : 0, k1 = fast1 ? 1 : 0;
-    if (slow0 | slow1) {
-        if (slow0) {
+    // bits 0, 1: the source needs the exact path; bits 2, 3: it was evaluated here, bits 4, 5: softened (counters)
+    return (slow0 ? 1u : 0u) | (slow1 ? 2u : 0u) | (COUNT ? ((fast0 ? 4u : 0u) | (fast1 ? 8u : 0u)) : 0u);
+}
+
+// The exact path of the sources flagged by eval_two_fast, and the counters.
+template <bool POT, bool COUNT>
+__device__ __forceinline__ void eval_two_slow(WarpSmem &w, const uint32_t flags, const float4 q0, const float4 q1,
+                                              const uint32_t e0, const uint32_t e1, const Target &t, const WalkConst &c,
+                                              Accum2 &acc, unsigned long long *cnt, LaneCount &lc)
+{
+    int k0 = (flags & 4u) ? ((flags & 16u) ? 2 : 1) : 0, k1 = (flags & 8u) ? ((flags & 32u) ? 2 : 1) : 0;
+    if (flags & 3u) {
+        if (flags & 1u) {
             const float4 d = pair_exact<POT>(q0, w.ring_h[e0], t, c, cnt, k0);
             acc2_add(acc.ax, d.x); acc2_add(acc.ay, d.y); acc2_add(acc.az, d.z); acc2_add(acc.pot, -d.w);
         }
-        if (slow1) {
+        if (flags & 2u) {
             const float4 d = pair_exact<POT>(q1, w.ring_h[e1], t, c, cnt, k1);
             acc2_add(acc.ax, d.x); acc2_add(acc.ay, d.y); acc2_add(acc.az, d.z); acc2_add(acc.pot, -d.w);
         }
     }
     if (COUNT) {
+        const bool v0 = e0 != GW_DUMMY, v1 = e1 != GW_DUMMY;
         const bool part0 = (w.seg_flags[(e0 >> 5) & (GW_NSEG - 1)] & SEG_PART) != 0u;
         const bool part1 = (w.seg_flags[(e1 >> 5) & (GW_NSEG - 1)] & SEG_PART) != 0u;
         if (v0) { if (part0) { lc.pin += (k0 != 0); lc.psoft += (k0 == 2); lc.pout += (k0 == 0); } else lc.ain += (k0 != 0); }
         if (v1) { if (part1) { lc.pin += (k1 != 0); lc.psoft += (k1 == 2); lc.pout += (k1 == 0); } else lc.ain += (k1 != 0); }
     }
+}
+
+template <bool POT, bool COUNT, bool WRAP, bool HLOOK>
+__device__ __forceinline__ void eval_two(WarpSmem &w, const float4 q0, const float4 q1, const uint32_t e0, const uint32_t e1,
+                                         const Target &t, const float hmax2g, const WalkConst &c, Accum2 &acc,
+                                         unsigned long long *cnt, LaneCount &lc)
+{
+    const uint32_t fl = eval_two_fast<POT, COUNT, WRAP, HLOOK>(w, q0, q1, e0, e1, t, hmax2g, c, acc);
+    eval_two_slow<POT, COUNT>(w, fl, q0, q1, e0, e1, t, c, acc, cnt, lc);
 }
 
 // Evaluates ring sources until every lane has finished all segments < target (tail <= target <= head; head =
@@ -456,31 +522,22 @@ __device__ __forceinline__ uint32_t consume(WarpSmem &w, const uint32_t head, co
         if (sg >= lp.nxt) need += k;
     }
     const uint32_t steps = __reduce_max_sync(0xffffffffu, need);
-#if OG_CONSUME_PIPELINED
-    if (steps != 0u) {
-        lp.nw = w.W[lp.nxt & (GW_NSEG - 1)][lane];
+    lp.nw = w.W[lp.nxt & (GW_NSEG - 1)][lane];
+#if OG_CONSUME_FOUR
+    // two takes per iteration: two independent packed chains for the scheduler to interleave
+    for (uint32_t it = 0u; it < steps; it += 2u) {
         uint32_t e0, e1, f0, f1;
         take_two(w, lp, head, lane, e0, e1);
-        float4 q0 = w.ring_pos[e0], q1 = w.ring_pos[e1], p0, p1;
-        uint32_t it = 1u;
-        for (; it + 1u < steps; it += 2u) {
-            take_two(w, lp, head, lane, f0, f1);
-            p0 = w.ring_pos[f0]; p1 = w.ring_pos[f1];
-            eval_two<POT, COUNT, WRAP, HLOOK>(w, q0, q1, e0, e1, t, hmax2g, c, acc, cnt, lc);
-            take_two(w, lp, head, lane, e0, e1);
-            q0 = w.ring_pos[e0]; q1 = w.ring_pos[e1];
-            eval_two<POT, COUNT, WRAP, HLOOK>(w, p0, p1, f0, f1, t, hmax2g, c, acc, cnt, lc);
+        take_two(w, lp, head, lane, f0, f1);
+        const float4 q0 = w.ring_pos[e0], q1 = w.ring_pos[e1], p0 = w.ring_pos[f0], p1 = w.ring_pos[f1];
+        const uint32_t fa = eval_two_fast<POT, COUNT, WRAP, HLOOK>(w, q0, q1, e0, e1, t, hmax2g, c, acc);
+        const uint32_t fb = eval_two_fast<POT, COUNT, WRAP, HLOOK>(w, p0, p1, f0, f1, t, hmax2g, c, acc);
+        if (COUNT || ((fa | fb) & 3u)) {
+            eval_two_slow<POT, COUNT>(w, fa, q0, q1, e0, e1, t, c, acc, cnt, lc);
+            eval_two_slow<POT, COUNT>(w, fb, p0, p1, f0, f1, t, c, acc, cnt, lc);
         }
-        if (it < steps) {
-            take_two(w, lp, head, lane, f0, f1);
-            p0 = w.ring_pos[f0]; p1 = w.ring_pos[f1];
-            eval_two<POT, COUNT, WRAP, HLOOK>(w, q0, q1, e0, e1, t, hmax2g, c, acc, cnt, lc);
-            q0 = p0; q1 = p1; e0 = f0; e1 = f1;
-        }
-        eval_two<POT, COUNT, WRAP, HLOOK>(w, q0, q1, e0, e1, t, hmax2g, c, acc, cnt, lc);
     }
 #else
-    lp.nw = w.W[lp.nxt & (GW_NSEG - 1)][lane];
     for (uint32_t it = 0u; it < steps; ++it) {
         uint32_t e0, e1;
         take_two(w, lp, head, lane, e0, e1);
@@ -559,7 +616,9 @@ k_walk_group(const __grid_constant__ WalkArgs a)
             if (loz >= halfL) { t.z -= c.L; g.gcz = 0.5f * ((loz - c.L) + (hiz - c.L)); }
         }
         // lanes whose target is the same sorted slot (duplicates in active_idx; the mirrored tail lanes)
-        const uint32_t peers = __match_any_sync(0xffffffffu, t.slot) & TMASK;   // as a target mask
+        // (as a target mask; with the identity list every valid lane has its own slot, and the mirrored tail lanes
+        // never appear in a mask)
+        const uint32_t peers = a.tgt_slot ? (__match_any_sync(0xffffffffu, t.slot) & TMASK) : mybit;
         const float hi2 = t.h * t.h;
         Accum2 acc2 = {0ull, 0ull, 0ull, 0ull};
         LaneCount lc = {0, 0, 0, 0, 0, 0};
@@ -680,8 +739,9 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                     uint32_t openw = 0u, sloww = 0u;
                     const uint32_t np = (nX + 1u) >> 1;
                     const f32x2 tx2 = bc2(t.x), ty2 = bc2(t.y), tz2 = bc2(t.z), A2 = bc2(GEOM ? c.theta2 : t.A);
+                    uint32_t bit0 = 1u << (2u * sl);   // bit of the pair's first node (the second one is the next bit)
 #pragma unroll 2
-                    for (uint32_t p = sl; p < np; p += (uint32_t)K) {
+                    for (uint32_t p = sl; p < np; p += (uint32_t)K, bit0 <<= 2 * K) {
                         const float4 a0 = w.xq[p][0], a1 = w.xq[p][1], a2 = w.xq[p][2], a3 = w.xq[p][3];
                         f32x2 dx = sub2(pk2(a0.x, a0.y), tx2), dy = sub2(pk2(a0.z, a0.w), ty2), dz = sub2(pk2(a1.x, a1.y), tz2);
                         if (xwrap) {
@@ -695,7 +755,7 @@ k_walk_group(const __grid_constant__ WalkArgs a)
                         float r20, r21, rh0, rh1;
                         upk2(r2, r20, r21);
                         upk2(rhs, rh0, rh1);
-                        const uint32_t bit0 = 1u << (2u * p), bit1 = 2u << (2u * p);
+                        const uint32_t bit1 = bit0 + bit0;
                         const bool in0 = (__float_as_uint(a3.z) & mybit) != 0u, in1 = (__float_as_uint(a3.w) & mybit) != 0u;
                         const bool cand0 = in0 && !(r20 > a1.z), cand1 = in1 && !(r21 > a1.w);
                         const bool fopen0 = rh0 < a2.x, fopen1 = rh1 < a2.y;
