@@ -116,7 +116,10 @@ typedef enum {
     OG_F_NODE_CELL = 11,    /* f32 [n_nodes][4]  (c_x, c_y, c_z, l)                        */
     OG_F_NODE_LO = 12,      /* f32 [n_nodes][4]  (lo_x, lo_y, lo_z, h_max)  tight AABB     */
     OG_F_NODE_HI = 13,      /* f32 [n_nodes][4]  (hi_x, hi_y, hi_z, unused)                */
-    OG_F_LEVEL_START = 14   /* u32 [23]    node index where each level starts (BFS)        */
+    OG_F_LEVEL_START = 14,  /* u32 [23]    node index where each level starts (BFS)        */
+    OG_F_WALK_COST = 15     /* u32 [n]     OG_COUNT trees only: interactions (accepted nodes + particle pairs)
+                               evaluated for each target of the LAST walk, in the caller's active order (the first
+                               n_active entries); the per-target work figure a host code balances its next step by */
 } og_field;
 
 /* Bytes of DEVICE workspace og_tree_build needs for n particles (0 on invalid input).    */
@@ -151,8 +154,11 @@ og_tree *og_tree_build(const float *pos, const float *mass, const float *soft, u
  *   pot_out    DEVICE f32 [n_active], overwritten, or NULL
  * Returns OG_OK or a negative og_status; conditions detected on the device (bad index, traversal stack
  * capacity) are latched and reported by og_tree_status().  n_active == 0 is a no-op.  Implementation note:
- * 32 targets per warp; an active subset of fewer than n / 16 targets is walked with 8 targets per warp
- * (4 lanes per target).  Results do not depend on the launch order (bit-reproducible run to run).
+ * the targets are taken in Morton order, 32 per warp; an active list that fills fewer than 1 / 16 of the Morton
+ * range it covers is walked with 8 targets per warp (4 lanes per target), decided on the device.  Results do not
+ * depend on the launch order (bit-reproducible run to run), and a call on a sub-list that covers whole warps of
+ * the full list's order (a multiple of 32 consecutive targets of the sorted active list) returns the same bits as
+ * the full call does for those targets.
  */
 int og_shortrange_accel(const og_tree *tree, const uint32_t *active_idx, uint64_t n_active,
                         const float *a_old, float *acc_out, float *pot_out, og_stream stream);

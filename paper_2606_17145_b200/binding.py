@@ -30,13 +30,13 @@ OG_COUNT = 4
 # og_field
 (OG_F_KEYS_SORTED, OG_F_PERM, OG_F_INV_PERM, OG_F_SPOS, OG_F_SH, OG_F_NODE_LEVEL, OG_F_NODE_FIRST,
  OG_F_NODE_COUNT, OG_F_NODE_FIRST_CHILD, OG_F_NODE_NCHILD, OG_F_NODE_COM, OG_F_NODE_CELL, OG_F_NODE_LO,
- OG_F_NODE_HI, OG_F_LEVEL_START) = range(15)
+ OG_F_NODE_HI, OG_F_LEVEL_START, OG_F_WALK_COST) = range(16)
 
 _FIELD_DTYPE = {
     OG_F_KEYS_SORTED: ("<u8", 8), OG_F_PERM: ("<u4", 4), OG_F_INV_PERM: ("<u4", 4), OG_F_SPOS: ("<f4", 4),
     OG_F_SH: ("<f4", 4), OG_F_NODE_LEVEL: ("|u1", 1), OG_F_NODE_FIRST: ("<u4", 4), OG_F_NODE_COUNT: ("<u4", 4),
     OG_F_NODE_FIRST_CHILD: ("<u4", 4), OG_F_NODE_NCHILD: ("|u1", 1), OG_F_NODE_COM: ("<f4", 4),
-    OG_F_NODE_CELL: ("<f4", 4), OG_F_NODE_LO: ("<f4", 4), OG_F_NODE_HI: ("<f4", 4), OG_F_LEVEL_START: ("<u4", 4),
+    OG_F_NODE_CELL: ("<f4", 4), OG_F_NODE_LO: ("<f4", 4), OG_F_NODE_HI: ("<f4", 4), OG_F_LEVEL_START: ("<u4", 4), OG_F_WALK_COST: ("<u4", 4),
 }
 
 

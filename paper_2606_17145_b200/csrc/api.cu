@@ -27,10 +27,10 @@ inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 struct Layout {
     size_t keysA, keysB, idxA, idxB, sort_scratch, spos, sh, inv_perm;
     size_t level, first, count, first_child, nchild, com, cell, lo, hi, info, rec;
-    size_t oct_scratch, level_start, status, counters, small_end, spill, total;
+    size_t oct_scratch, level_start, status, counters, small_end, spill, cost, total;
 };
 
-Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count, uint32_t spill_entries)
+Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count, uint32_t spill_entries, bool count)
 {
     Layout L;
     size_t o = 0;
@@ -51,6 +51,7 @@ Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count, uint32_t spill_
     L.counters = take(OGC_N * 8);
     L.small_end = o;
     L.spill = take(ogk_walk_spill_bytes(sm_count, spill_entries));
+    L.cost = take(count ? n * 4 : 0);
     L.total = o;
     return L;
 }
@@ -178,7 +179,7 @@ extern "C" size_t og_tree_workspace_bytes(uint64_t n, const og_params *params)
     if (!params || params->struct_size != sizeof(og_params) || n == 0 || n >= (1ull << 31)) return 0;
     int sms = device_sm_count(nullptr);
     if (sms <= 0) sms = 148;  // no device visible: size for a B200
-    return make_layout(n, default_max_nodes(n, params), sms, ogk_walk_spill_entries(params)).total;
+    return make_layout(n, default_max_nodes(n, params), sms, ogk_walk_spill_entries(params), (params->flags & OG_COUNT) != 0).total;
 }
 
 // og_tree_build; `before_gather` (may be NULL) is awaited on the stream before mass / soft are first read
@@ -208,7 +209,7 @@ static og_tree *tree_build_impl(const float *pos, const float *mass, const float
         delete t;
         return nullptr;
     }
-    const Layout L = make_layout(n, t->max_nodes, sms, t->walk_spill_cap);
+    const Layout L = make_layout(n, t->max_nodes, sms, t->walk_spill_cap, (params->flags & OG_COUNT) != 0);
     if (params->workspace) {
         if (params->workspace_bytes < L.total || ((uintptr_t)params->workspace & 255u)) {
             og_set_error("workspace too small or not 256-byte aligned: %zu bytes given, %zu needed",
@@ -240,6 +241,7 @@ static og_tree *tree_build_impl(const float *pos, const float *mass, const float
     t->node_rec = (uint4 *)(b + L.rec);
     t->d_level_start = (uint32_t *)(b + L.level_start); t->d_status = (uint32_t *)(b + L.status);
     t->d_counters = (unsigned long long *)(b + L.counters);
+    t->walk_cost = (params->flags & OG_COUNT) ? (uint32_t *)(b + L.cost) : nullptr;
     t->walk_spill = b + L.spill; t->walk_spill_bytes = ogk_walk_spill_bytes(sms, t->walk_spill_cap);
 
 #define OG_BUILD_TRY(expr)                                                    \
@@ -312,7 +314,7 @@ extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx,
 #define OG_ACC_TRY(expr) OG_CUDA_TRY(expr, { cudaFreeAsync(tmp, st); return OG_ERR_CUDA; })
     OG_ACC_TRY(ogk_active_slots(active_idx, t->inv_perm, t->n, n_active, k0, v0, t->d_status, st));
     OG_ACC_TRY(ogk_radix_sort(k0, v0, k1, v1, n_active, 0, bits, tmp + o_sc, &in_alt, st));
-    OG_ACC_TRY(ogk_unpack_slots(in_alt ? k1 : k0, n_active, slots, st));
+    OG_ACC_TRY(ogk_unpack_slots(in_alt ? k1 : k0, n_active, slots, OG_SPARSE_DIV, t->d_status + 2, st));
     OG_ACC_TRY(ogk_walk(t, slots, in_alt ? v1 : v0, n_active, a_old, acc_out, pot_out, st));
     OG_ACC_TRY(cudaEventRecord(t->ev_walked, st));
     t->walked = true;
@@ -346,6 +348,9 @@ extern "C" int og_tree_get(const og_tree *t, int field, const void **dev_ptr, ui
     case OG_F_NODE_LO: *dev_ptr = t->node_lo; *count = nn * 4; break;
     case OG_F_NODE_HI: *dev_ptr = t->node_hi; *count = nn * 4; break;
     case OG_F_LEVEL_START: *dev_ptr = t->d_level_start; *count = 23; break;
+    case OG_F_WALK_COST:
+        if (!t->walk_cost) { og_set_error("OG_F_WALK_COST needs a tree built with OG_COUNT"); return OG_ERR_INVALID_ARG; }
+        *dev_ptr = t->walk_cost; *count = t->n; break;
     default: og_set_error("unknown field %d", field); return OG_ERR_INVALID_ARG;
     }
     return OG_OK;

@@ -129,12 +129,21 @@ k_active_slots(const uint32_t *__restrict__ active_idx, const uint32_t *__restri
     vals[t] = (uint32_t)t;
 }
 
+// Also decides (on the device: no host round trip) how the walk groups these targets: `*sparse` = 1 if the active
+// targets fill fewer than 1 / sparse_div of the sorted slots between the first and the last of them (the walk then
+// takes 8 targets per warp), else 0.  The density is that of the Morton range the list covers, so a contiguous range
+// of a larger set (one rank's share, a spatial region) is walked like the full set.
 __global__ void __launch_bounds__(256)
-k_unpack_slots(const uint64_t *__restrict__ keys, uint64_t n_active, uint32_t *__restrict__ slots)
+k_unpack_slots(const uint64_t *__restrict__ keys, uint64_t n_active, uint32_t *__restrict__ slots, uint32_t sparse_div,
+               uint32_t *__restrict__ sparse)
 {
     const uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n_active) return;
     slots[t] = (uint32_t)keys[t];
+    if (t == 0) {
+        const uint64_t span = keys[n_active - 1] - keys[0] + 1;
+        *sparse = (n_active * (uint64_t)sparse_div < span) ? 1u : 0u;
+    }
 }
 
 cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_perm, uint64_t n,
@@ -146,9 +155,10 @@ cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_per
     return cudaGetLastError();
 }
 
-cudaError_t ogk_unpack_slots(const uint64_t *keys, uint64_t n_active, uint32_t *slots, cudaStream_t st)
+cudaError_t ogk_unpack_slots(const uint64_t *keys, uint64_t n_active, uint32_t *slots, uint32_t sparse_div,
+                             uint32_t *sparse, cudaStream_t st)
 {
     const unsigned grid = (unsigned)((n_active + 255) / 256);
-    k_unpack_slots<<<grid, 256, 0, st>>>(keys, n_active, slots);
+    k_unpack_slots<<<grid, 256, 0, st>>>(keys, n_active, slots, sparse_div, sparse);
     return cudaGetLastError();
 }

@@ -68,7 +68,8 @@ struct og_tree {
     uint4 *node_rec;           // [3 n_nodes]: n0, n1, n2 of node j at 3 j, 3 j + 1, 3 j + 2 (48 contiguous bytes)
     // small device state
     uint32_t *d_level_start;   // [24]: start index per level, [22] = n_nodes, [23] = max level
-    uint32_t *d_status;        // [4]: latched status bits, walk work counter, ...
+    uint32_t *d_status;        // [16]: [0] latched status bits, [1] walk work counter, [2] sparse-active-list flag
+    uint32_t *walk_cost;       // [n] OG_COUNT only: interactions evaluated per target of the last walk, caller's order
     unsigned long long *d_counters;  // [OGC_N]
     // walk scratch (spill stacks), allocated lazily
     void *walk_spill;
@@ -122,4 +123,6 @@ uint32_t ogk_walk_spill_entries(const og_params *p);
 cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_perm, uint64_t n,
                              uint64_t n_active, uint64_t *keys, uint32_t *vals, uint32_t *d_status,
                              cudaStream_t st);
-cudaError_t ogk_unpack_slots(const uint64_t *keys, uint64_t n_active, uint32_t *slots, cudaStream_t st);
+cudaError_t ogk_unpack_slots(const uint64_t *keys, uint64_t n_active, uint32_t *slots, uint32_t sparse_div,
+                             uint32_t *sparse, cudaStream_t st);
+#define OG_SPARSE_DIV 16u  // an active list that fills fewer than 1 / 16 of its Morton range counts as sparse (8 targets per warp)

@@ -43,6 +43,9 @@ struct WalkArgs {
     uint32_t *spill;
     uint32_t spill_cap;        // entries per warp
     uint32_t stack_cap;        // ranges kept in shared memory before half of them are spilled (<= GW_STACK, even)
+    const uint32_t *sel_flag;  // device flag: this launch runs iff *sel_flag == sel (NULL: always); see launch()
+    uint32_t sel;
+    uint32_t *cost;            // OG_COUNT: interactions evaluated per target (caller's order), or NULL
     WalkConst c;
 };
 
@@ -82,9 +85,6 @@ __device__ __forceinline__ Target load_target(const WalkArgs &a, uint32_t k, uin
 #endif
 #ifndef OG_GW_SPARSE_G
 #define OG_GW_SPARSE_G 8   // targets per warp for sparse active subsets (4, 8 or 16; zoom: 31.9 / 31.3 / 36.7 ms)
-#endif
-#ifndef OG_SPARSE_DIV
-#define OG_SPARSE_DIV 16u  // an active subset of fewer than n / 16 targets counts as sparse (10 % active: 77 ms at 32 per warp, 101 ms at 8)
 #endif
 #ifndef OG_GW_STACK
 #define OG_GW_STACK 256
@@ -568,6 +568,7 @@ k_walk_group(const __grid_constant__ WalkArgs a)
     const uint32_t mybit = 1u << tl;                          // in target masks
     const uint32_t myslots = SLICE0 << sl;                    // the slots this lane evaluates
     const WalkConst &c = a.c;
+    if (a.sel_flag != nullptr && __ldg(a.sel_flag) != a.sel) return;   // the other instantiation was chosen
     unsigned long long *cnt = COUNT ? a.counters : nullptr;
     uint32_t *sp_start = a.spill + (size_t)(blockIdx.x * GW_WARPS + wid) * 3 * a.spill_cap;
     uint32_t *sp_cnt = sp_start + a.spill_cap, *sp_mask = sp_cnt + a.spill_cap;
@@ -938,6 +939,14 @@ k_walk_group(const __grid_constant__ WalkArgs a)
             a.acc_out[3 * (size_t)out + 2] = acc.az;
             if (POT) a.pot_out[out] = acc.pot;
         }
+        if (COUNT && a.cost != nullptr) {   // per-target work figure (OG_F_WALK_COST): interactions evaluated
+            uint32_t wk = lc.ain + lc.pin + lc.pout;
+            if (G < 32) {
+#pragma unroll
+                for (int o = G; o < 32; o <<= 1) wk += __shfl_xor_sync(0xffffffffu, wk, o);
+            }
+            if (valid && sl == 0u) a.cost[out] = wk;
+        }
         if (COUNT) {
             const uint32_t v[6] = {lc.full, lc.cull, lc.ain, lc.pin, lc.psoft, lc.pout};
             const int slot[6] = {OGC_V_FULL, OGC_V_CULL, OGC_A_IN, OGC_P_IN, OGC_P_SOFT, OGC_P_OUT};
@@ -950,17 +959,12 @@ k_walk_group(const __grid_constant__ WalkArgs a)
     }
 }
 
-template <bool GEOM, bool POT, bool COUNT>
-cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
+template <bool GEOM, bool POT, bool COUNT, int G>
+cudaError_t launch_g(const og_tree *t, WalkArgs a, cudaStream_t st)
 {
-    // Targets per warp: 32 when the active targets are dense in Morton order; 8 (4 lanes per target) for a
-    // sparse active subset, whose 32 consecutive targets would span many cells (zoom: 52 -> 31 ms).  For the
-    // spread-out groups of a DENSE target set (uniform background of nfw256) 8 per warp is slower (measured).
-    const bool sparse = a.tgt_slot != nullptr && (uint64_t)a.n_active * OG_SPARSE_DIV < t->n;
-    const int G = sparse ? OG_GW_SPARSE_G : 32;
     a.n_groups = (uint32_t)(((uint64_t)a.n_active + G - 1) / G);
     const size_t smem = GW_WARPS * sizeof(WarpSmem);
-    auto kern = sparse ? k_walk_group<GEOM, POT, COUNT, OG_GW_SPARSE_G> : k_walk_group<GEOM, POT, COUNT, 32>;
+    auto kern = k_walk_group<GEOM, POT, COUNT, G>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
@@ -971,6 +975,26 @@ cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
     const unsigned grid = (unsigned)(per_sm * t->sm_count);
     kern<<<grid, GW_THREADS, smem, st>>>(a);
     return cudaGetLastError();
+}
+
+// Targets per warp: 32 when the active targets are dense in Morton order; 8 (4 lanes per target) for a sparse active
+// list, whose 32 consecutive targets would span many cells (zoom: 52 -> 21 ms).  For the spread-out groups of a DENSE
+// target set (uniform background of nfw256) 8 per warp is slower (measured).  With an explicit active list the choice
+// is made on the device from the density of the list in the Morton range it covers (k_unpack_slots): both
+// instantiations are launched and the one that was not chosen returns at once (no host round trip).
+template <bool GEOM, bool POT, bool COUNT>
+cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
+{
+    if (a.tgt_slot == nullptr) {
+        a.sel_flag = nullptr; a.sel = 0u;
+        return launch_g<GEOM, POT, COUNT, 32>(t, a, st);
+    }
+    a.sel_flag = t->d_status + 2;
+    a.sel = 0u;
+    cudaError_t e = launch_g<GEOM, POT, COUNT, 32>(t, a, st);
+    if (e != cudaSuccess) return e;
+    a.sel = 1u;
+    return launch_g<GEOM, POT, COUNT, OG_GW_SPARSE_G>(t, a, st);
 }
 
 }  // namespace
@@ -998,6 +1022,7 @@ cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t 
     a.status = t->d_status;
     a.counters = t->d_counters;
     a.spill = reinterpret_cast<uint32_t *>(t->walk_spill);
+    a.cost = t->walk_cost;
     a.spill_cap = t->walk_spill_cap;
     a.stack_cap = t->prm.walk_stack_entries ? min(t->prm.walk_stack_entries, (uint32_t)GW_STACK) : (uint32_t)GW_STACK;
     const og_params &p = t->prm;

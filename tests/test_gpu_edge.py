@@ -297,3 +297,40 @@ def test_walks_on_other_streams_are_ordered_after_build_and_each_other(B):
         assert torch.equal(a1, a_ref) and torch.equal(p1, p_ref)
         assert torch.equal(a2, a_ref2) and torch.equal(p2, p_ref2)
     B.og_trim()
+
+
+# ---- sub-lists, device-side grouping decision, per-target work figure -------------------------------------
+def test_sublist_of_whole_warps_returns_the_same_bits_and_cost_field(B):
+    """og.h: a call on a sub-list that covers whole warps (multiples of 32 consecutive targets) of the sorted active
+    order returns the same bits as the full call -- also when the sub-list is a small part of the box (the grouping is
+    decided from the density of the list in ITS Morton range, not from n_active / n).  With OG_COUNT the tree also
+    records the interactions evaluated per target (OG_F_WALK_COST), whose sum is A_in + P_in + P_out."""
+    import torch
+    w = W.make("nfw256", small=True)
+    pos, mass, eps = (torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps))
+    prm = B.make_params(w.r_s, G=w.G, alpha=w.alpha, theta=w.theta, flags=B.OG_PERIODIC | B.OG_COUNT)
+    tree = B.og_tree_build(pos, mass, eps, w.L, prm)
+    a_full, p_full = B.og_shortrange_accel(tree, None, None)
+    st = B.og_tree_stats(tree)
+    cost = B.og_tree_get(tree, B.OG_F_WALK_COST).cpu().numpy().view(np.uint32)
+    assert int(cost.astype(np.int64).sum()) == st["A_in"] + st["P_in"] + st["P_out"]
+    assert cost.min() > 0
+    perm = B.og_tree_get(tree, B.OG_F_PERM).cpu().numpy().view(np.uint32)
+    n = w.n
+    for lo, hi in ((0, 32 * 5), (32 * 100, 32 * 163), (n - (n % 32) - 64, n)):      # the last one includes the ragged tail
+        sub = perm[lo:hi].copy()
+        rng = np.random.default_rng(lo)
+        rng.shuffle(sub)                                                        # any order: the library sorts by slot
+        act = torch.from_numpy(sub.view(np.int32)).cuda()
+        a_sub, p_sub = B.og_shortrange_accel(tree, act, None)
+        idx = torch.from_numpy(sub.astype(np.int64)).cuda()
+        assert torch.equal(a_sub, a_full[idx]) and torch.equal(p_sub, p_full[idx]), (lo, hi)
+        c2 = B.og_tree_get(tree, B.OG_F_WALK_COST).cpu().numpy().view(np.uint32)[: hi - lo]
+        assert np.array_equal(c2, cost[sub])
+    assert B.og_tree_status(tree) == B.OG_OK
+    B.og_tree_free(tree)
+    # a tree built without OG_COUNT has no such field
+    tree = B.og_tree_build(pos, mass, eps, w.L, B.make_params(w.r_s))
+    with pytest.raises(B.OgError):
+        B.og_tree_get(tree, B.OG_F_WALK_COST)
+    B.og_tree_free(tree)
