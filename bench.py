@@ -275,7 +275,8 @@ def run_ours(args):
     world, rank, local = dist_setup(args.gpus, "nccl")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    w = make_workload(args.workload, rank)
+    strong = args.scaling == "strong"
+    w = make_workload(args.workload, 0 if strong else rank)   # strong: every rank holds the same box (and tree)
     n, na = w.n, w.n_active
     prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8)
     h_pos = torch.from_numpy(w.pos).pin_memory()
@@ -295,6 +296,33 @@ def run_ours(args):
         raise SystemExit("bench.py: tree status " + B.og_last_error())
     st_tree = B.og_tree_stats(tree)
     B.og_tree_free(tree)
+
+    shard = None
+    if strong:
+        # SURVEY.md Sec. 8.5 / DESIGN.md Sec. 8: redundant tree per rank, contiguous Morton range of the active targets per
+        # rank, balanced by the per-target work of an (untimed) counted pass; no data-path collective, no reduction
+        from paper_2606_17145_b200 import sharding as S
+        prm_c = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8,
+                              flags=B.OG_PERIODIC | B.OG_COUNT)
+        tc = B.og_tree_build(pos, mass, eps, w.L, prm_c)
+        B.og_shortrange_accel(tc, act, a_old, acc_out=acc, pot_out=pot)
+        torch.cuda.synchronize()
+        cost = B.og_tree_get(tc, B.OG_F_WALK_COST).cpu().numpy().view(np.uint32)[:na]
+        inv_perm = B.og_tree_get(tc, B.OG_F_INV_PERM).cpu().numpy().view(np.uint32)
+        B.og_tree_free(tc)
+        slots = inv_perm if w.active_idx is None else inv_perm[w.active_idx]
+        order = S.sorted_active_order(slots)
+        bounds = S.partition_by_cost(cost[order], world)
+        my_pos, my_idx = S.rank_sublist(w.active_idx, n, order, bounds, rank)
+        full_acc, full_pot = acc.clone(), pot.clone()                 # the single-call result, for the bit check below
+        my_pos_d = torch.from_numpy(my_pos.astype(np.int64)).to(dev)
+        act = torch.from_numpy(my_idx.view(np.int32)).to(dev)
+        a_old = a_old[my_pos_d].contiguous()
+        na = int(my_idx.shape[0])
+        acc = torch.empty((na, 3), dtype=torch.float32, device=dev)
+        pot = torch.empty((na,), dtype=torch.float32, device=dev)
+        shard = {"bounds": [int(x) for x in bounds], "cost_share_max_over_mean":
+                 float(max(cost[order][bounds[r]:bounds[r + 1]].sum() for r in range(world)) * world / max(cost.sum(), 1))}
 
     def step(ev=None):
         if ev:
@@ -333,6 +361,12 @@ def run_ours(args):
     n_act_all = all_gather_int(na, dev)
     value = aggregate(n_act_all, ms_step)
 
+    if strong:
+        # every rank's share equals the single-call result bit for bit (whole warps of the same sorted order)
+        ok = bool(torch.equal(acc, full_acc[my_pos_d]) and torch.equal(pot, full_pot[my_pos_d]))
+        shard["bitwise_equal_to_single_call"] = bool(all_max(0.0 if ok else 1.0, dev) == 0.0)
+        h_act = torch.from_numpy(my_idx.view(np.int32)).pin_memory()
+        del full_acc, full_pot
     # e2e through the HOST-buffer entry point (pinned inputs, H2D + build + walk + D2H inside)
     h_aold = a_old.cpu().pin_memory()
     h_acc = torch.empty((na, 3), dtype=torch.float32).pin_memory()
@@ -400,12 +434,15 @@ def run_ours(args):
     }
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": w.name, "n": n, "n_active": na, "box": w.L, "r_s": w.r_s, "alpha": w.alpha,
+        "config": {"workload": w.name, "n": n, "n_active": int(sum(n_act_all)) if strong else na, "box": w.L, "r_s": w.r_s, "alpha": w.alpha,
                    "leaf_max": 8, "n_nodes": st_tree["n_nodes"], "max_level": st_tree["max_level"],
                    "l2_policy": "inputs larger than L2 (no flush): particles + tree > 1.5 GB vs 126 MB L2",
-                   "parallelism": f"{world} independent boxes (one per GPU)" if world > 1 else "1 GPU"},
+                   "parallelism": ("1 GPU" if world == 1 else
+                                   f"{world} GPUs, one box: tree built on every rank, Morton ranges of the active targets "
+                                   f"balanced by last pass's per-target work" if strong else
+                                   f"{world} independent boxes (one per GPU)")},
         "clocks": clocks,
         "e2e": {"value": aggregate(n_act_all, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e, "steps": e2e_steps},
@@ -416,6 +453,8 @@ def run_ours(args):
         "interactions_per_s_walk_only": inter / (ms_walk * 1e-3),
         "walk_counters": stc, "status": status, "checksum_mean_abs_acc": checksum,
     }
+    if shard is not None:
+        line["strong_sharding"] = shard
     if world == 1 and not args.no_cpu_baseline:
         cb, _ = cpu_baseline(w, sample=args.cpu_sample)
         line["cpu_baseline"] = cb
@@ -433,6 +472,9 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1 << 17)
     ap.add_argument("--ref-sample", type=int, default=1 << 15)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak (default): one independent box per GPU; strong: one box, every rank builds the tree and walks "
+                         "a Morton range of the active targets (SURVEY.md Sec. 8.5)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3 if args.impl == "ours" else args.warmup
