@@ -2,11 +2,12 @@
 // pairs, 8 bits per pass (C2, R3).  Stability is what delivers the index tie-break: the
 // values start as the identity, so equal keys stay in ascending original index.
 //
-// Per pass (HBM-bound): k_hist reads the keys of each 4096-key tile (8 B/key) and writes a
+// Per pass (HBM-bound): k_hist reads the keys of each 2048-key tile (8 B/key) and writes a
 // per-tile digit histogram; k_scan turns the digit-major histogram into global offsets;
 // k_scatter re-reads the tile (12 B/pair), ranks every key inside its tile in input order
-// (warp match-any ranking, per-warp digit counters in shared memory) and writes the pair to
-// its final place (12 B/pair).  32 B/pair/pass.
+// (nine ballots give the lanes with an equal digit, per-warp digit counters in shared memory) and
+// writes the pair to its final place (12 B/pair).  32 B/pair/pass.  A pass sorts on the bits
+// [shift, shift + nbits) only (nbits < 8 in the last pass of a range that is not a multiple of 8).
 #include "og_internal.cuh"
 
 namespace {
@@ -14,8 +15,8 @@ namespace {
 constexpr int SORT_THREADS = 256;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
 constexpr int SORT_ITEMS = 8;                        // keys per thread
-constexpr int SORT_WARP_TILE = 32 * SORT_ITEMS;      // 512 consecutive keys per warp
-constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS; // 4096 keys per block
+constexpr int SORT_WARP_TILE = 32 * SORT_ITEMS;      // 256 consecutive keys per warp
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS; // 2048 keys per block
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
 // Lanes of the warp whose 8-bit digit equals this lane's (and whose `ok` flag equals this lane's): nine
@@ -42,7 +43,7 @@ __device__ __forceinline__ uint32_t lanemask_lt()
 
 // hist[d * n_tiles + tile] = number of keys of the tile whose digit is d; ghist[d] += same.
 __global__ void __launch_bounds__(SORT_THREADS)
-k_sort_hist(const uint64_t *__restrict__ keys, uint64_t n, int shift, uint32_t n_tiles,
+k_sort_hist(const uint64_t *__restrict__ keys, uint64_t n, int shift, uint32_t dmask, uint32_t n_tiles,
             uint32_t *__restrict__ hist, uint32_t *__restrict__ ghist)
 {
     __shared__ uint32_t h[256];
@@ -54,7 +55,7 @@ k_sort_hist(const uint64_t *__restrict__ keys, uint64_t n, int shift, uint32_t n
         const uint64_t i = base + (uint64_t)r * 32;
         {
             const bool ok = i < n;
-            const uint32_t d = ok ? ((uint32_t)(__ldg(keys + i) >> shift) & 255u) : 0u;
+            const uint32_t d = ok ? ((uint32_t)(__ldg(keys + i) >> shift) & dmask) : 0u;
             // aggregate equal digits inside the warp before touching shared memory
             const uint32_t peers = digit_peers(d, ok);
             if (ok && (peers & lanemask_lt()) == 0) atomicAdd(&h[d], __popc(peers));
@@ -109,8 +110,8 @@ k_sort_scan(uint32_t *__restrict__ hist, const uint32_t *__restrict__ ghist, uin
     }
 }
 
-// Stable scatter of one 4096-pair tile.  Every key is ranked inside the tile in input order (warp
-// match-any ranking, per-warp digit counters, exclusive prefix over the warps and over the digits),
+// Stable scatter of one 2048-pair tile.  Every key is ranked inside the tile in input order (ballot
+// ranking, per-warp digit counters, exclusive prefix over the warps and over the digits),
 // the tile is reordered by digit in shared memory, and then written out: consecutive threads write
 // consecutive elements of a digit's run, so the global stores are coalesced runs instead of 32
 // scattered 8-byte writes per warp instruction.
@@ -124,7 +125,7 @@ struct ScatterSmem {
 __global__ void __launch_bounds__(SORT_THREADS)
 k_sort_scatter(const uint64_t *__restrict__ keys_in, const uint32_t *__restrict__ vals_in,
                uint64_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out, uint64_t n,
-               int shift, uint32_t n_tiles, const uint32_t *__restrict__ offs)
+               int shift, uint32_t dmask, uint32_t n_tiles, const uint32_t *__restrict__ offs)
 {
     extern __shared__ __align__(16) unsigned char sort_smem_raw[];
     ScatterSmem &sm = *reinterpret_cast<ScatterSmem *>(sort_smem_raw);
@@ -147,12 +148,12 @@ k_sort_scatter(const uint64_t *__restrict__ keys_in, const uint32_t *__restrict_
         key[r] = ok ? __ldg(keys_in + i) : ~0ull;
         val[r] = ok ? __ldg(vals_in + i) : 0u;
     }
-    // rank inside the warp's 512-key chunk, in input order (round-major, lane-minor)
+    // rank inside the warp's 256-key chunk, in input order (round-major, lane-minor)
     const uint32_t lt = lanemask_lt();
 #pragma unroll
     for (int r = 0; r < SORT_ITEMS; ++r) {
         const bool ok = (base + (uint64_t)r * 32) < n;
-        const uint32_t d = ok ? ((uint32_t)(key[r] >> shift) & 255u) : 0u;
+        const uint32_t d = ok ? ((uint32_t)(key[r] >> shift) & dmask) : 0u;
         const uint32_t peers = digit_peers(d, ok);
         const int leader = __ffs(peers) - 1;
         uint32_t b = 0;
@@ -194,7 +195,7 @@ k_sort_scatter(const uint64_t *__restrict__ keys_in, const uint32_t *__restrict_
 #pragma unroll
     for (int r = 0; r < SORT_ITEMS; ++r) {
         if ((base + (uint64_t)r * 32) < n) {
-            const uint32_t d = (uint32_t)(key[r] >> shift) & 255u;
+            const uint32_t d = (uint32_t)(key[r] >> shift) & dmask;
             const uint32_t p = sm.cnt[wid][d] + rank[r];
             sm.keys[p] = key[r];
             sm.vals[p] = val[r];
@@ -207,7 +208,7 @@ k_sort_scatter(const uint64_t *__restrict__ keys_in, const uint32_t *__restrict_
         const uint32_t i = tid + r * SORT_THREADS;
         if (i < in_tile) {
             const uint64_t k = sm.keys[i];
-            const uint32_t p = sm.gbase[(uint32_t)(k >> shift) & 255u] + i;
+            const uint32_t p = sm.gbase[(uint32_t)(k >> shift) & dmask] + i;
             keys_out[p] = k;
             vals_out[p] = sm.vals[i];
         }
@@ -240,9 +241,11 @@ cudaError_t ogk_radix_sort(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, u
     uint32_t *vin = vals, *vout = vals_alt;
     for (int p = 0; p < passes; ++p) {
         const int shift = begin_bit + 8 * p;
-        k_sort_hist<<<n_tiles, SORT_THREADS, 0, st>>>(kin, n, shift, n_tiles, hist, ghist + 256 * p);
+        const int nbits = (end_bit - shift) < 8 ? (end_bit - shift) : 8;     // the contract is [begin_bit, end_bit)
+        const uint32_t dmask = (1u << nbits) - 1u;
+        k_sort_hist<<<n_tiles, SORT_THREADS, 0, st>>>(kin, n, shift, dmask, n_tiles, hist, ghist + 256 * p);
         k_sort_scan<<<256, 1024, 0, st>>>(hist, ghist + 256 * p, n_tiles);
-        k_sort_scatter<<<n_tiles, SORT_THREADS, sizeof(ScatterSmem), st>>>(kin, vin, kout, vout, n, shift, n_tiles, hist);
+        k_sort_scatter<<<n_tiles, SORT_THREADS, sizeof(ScatterSmem), st>>>(kin, vin, kout, vout, n, shift, dmask, n_tiles, hist);
         uint64_t *tk = kin; kin = kout; kout = tk;
         uint32_t *tv = vin; vin = vout; vout = tv;
     }

@@ -82,6 +82,23 @@ def test_a2_radix_sort_partial_bits(B):
     assert np.array_equal(u32(vs), np.argsort(k, kind="stable").astype(np.uint32))
 
 
+@pytest.mark.parametrize("begin_bit,end_bit", [(0, 20), (3, 13), (5, 6), (40, 63)])
+def test_a2_radix_sort_sorts_on_the_stated_bits_only(B, begin_bit, end_bit):
+    """og.h: stable sort by the key bits [begin_bit, end_bit): bits above end_bit (and below begin_bit) are random
+    here and must not influence the order, also when the range is not a multiple of 8."""
+    import torch
+    n = 70_001
+    rng = np.random.default_rng(11)
+    k = rng.integers(0, 1 << 63, n, dtype=np.uint64)
+    kd = torch.from_numpy(k.view(np.int64)).cuda()
+    vd = torch.arange(n, dtype=torch.int32, device="cuda")
+    ks, vs = B.og_radix_sort_pairs(kd, vd, begin_bit, end_bit)
+    field = (k >> np.uint64(begin_bit)) & np.uint64((1 << (end_bit - begin_bit)) - 1)
+    ref = np.argsort(field, kind="stable").astype(np.uint32)
+    assert np.array_equal(u32(vs), ref)
+    assert np.array_equal(u64(ks), k[ref])
+
+
 # ---- a2..a5: permutation, topology, node records -------------------------------------------
 @pytest.mark.parametrize("name,leaf_max", [(n, 8) for n in SMALL[:5]] + [("nfw256", 1), ("nfw256", 32)])
 def test_tree_bit_exact(B, name, leaf_max):
