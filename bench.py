@@ -465,6 +465,78 @@ def run_ours(args):
     return 0
 
 
+def run_timesteps(args):
+    """--timesteps K (row f2): K synchronisation steps of the hierarchical time-step shell on the
+    workload (all particles, seeded small velocities): next tick -> drift ALL -> active list -> tree rebuild -> short-range
+    walk of the active particles with their carried a_old -> kick + new bins.  Prints its own JSON line: per-step sizes
+    of the active set and device times of each phase (the paper's small-bin regime)."""
+    import torch
+    from paper_2606_17145_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    w = W.make(args.workload)
+    n, L = w.n, w.L
+    prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8)
+    pos = torch.from_numpy(w.pos).to(dev)
+    mass, eps = torch.from_numpy(w.mass).to(dev), torch.from_numpy(w.eps).to(dev)
+    tree = B.og_tree_build(pos, mass, eps, L, prm)
+    acc, _ = B.og_shortrange_accel(tree, None, None, want_pot=False)
+    B.og_tree_free(tree)
+    anorm = torch.linalg.vector_norm(acc, dim=1)
+    a_med = float(anorm.median().item())
+    eta, bmax = 0.025, 8
+    dt_max = 4.0 * float(np.sqrt(2.0 * eta * float(w.eps.mean()) / a_med))     # the median particle sits two levels down
+    g = torch.Generator(device=dev)
+    g.manual_seed(W.SEED0 + 77)
+    vel = (torch.randn((n, 3), generator=g, device=dev) * (0.05 * float(w.eps.mean()) / (dt_max / 2 ** bmax) / 16)).contiguous()
+    bins = torch.zeros(n, dtype=torch.uint8, device=dev)
+    a_old = torch.zeros(n, device=dev)
+    act = torch.empty(n, dtype=torch.int32, device=dev)
+    scratch = torch.empty(B.og_ts_scratch_bytes(n), dtype=torch.uint8, device=dev)
+    B.og_ts_kick(vel, bins, a_old, None, n, acc, eps, eta, dt_max, bmax, 0, True)
+    hist0 = torch.bincount(bins.long(), minlength=bmax + 1).cpu().tolist()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    tick, rows = 0, []
+    torch.cuda.synchronize()
+    t_all0 = ev(); t_all1 = ev()
+    t_all0.record()
+    for _ in range(args.timesteps):
+        e = [ev() for _ in range(6)]
+        e[0].record()
+        nxt = B.og_ts_next_tick(bins, tick, bmax, scratch)
+        B.og_ts_drift(pos, vel, (nxt - tick) * dt_max / 2 ** bmax, L)
+        tick = nxt
+        e[1].record()
+        na = B.og_ts_active_list(bins, tick, bmax, act, scratch)
+        sub = act[:na]
+        ao = a_old[sub.long()].contiguous()
+        e[2].record()
+        tree = B.og_tree_build(pos, mass, eps, L, prm)
+        e[3].record()
+        acc, _ = B.og_shortrange_accel(tree, sub, ao, want_pot=False)
+        e[4].record()
+        B.og_ts_kick(vel, bins, a_old, sub, na, acc, eps, eta, dt_max, bmax, tick, False)
+        B.og_tree_free(tree)
+        e[5].record()
+        rows.append((tick, na, e))
+    t_all1.record()
+    torch.cuda.synchronize()
+    per = [{"tick": t, "n_active": na, "ms_drift": e[0].elapsed_time(e[1]), "ms_active_list": e[1].elapsed_time(e[2]),
+            "ms_build": e[2].elapsed_time(e[3]), "ms_walk": e[3].elapsed_time(e[4]), "ms_kick": e[4].elapsed_time(e[5])}
+           for t, na, e in rows]
+    total_ms = t_all0.elapsed_time(t_all1)
+    updates = sum(p["n_active"] for p in per)
+    line = {"mode": "timestep", "metric": "active-particle force updates/s over K hierarchical time steps (drift-all + tree "
+            "rebuild + short-range walk + kick) on B200", "value": updates / (total_ms * 1e-3), "unit": "particle updates/s",
+            "n_gpus": 1, "steps": args.timesteps, "ms_total": total_ms, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "n": n, "eta": eta, "dt_max": dt_max, "bmax": bmax, "initial_bin_histogram": hist0},
+            "per_step": per, "status": 0}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -478,7 +550,11 @@ def main():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="weak (default): one independent box per GPU; strong: one box, every rank builds the tree and walks "
                          "a Morton range of the active targets (SURVEY.md Sec. 8.5)")
+    ap.add_argument("--timesteps", type=int, default=0,
+                    help="row f2: run this many synchronisation steps of the time-step shell instead of the standard step")
     args = ap.parse_args()
+    if args.timesteps > 0:
+        return run_timesteps(args)
     if args.warmup < 3:
         args.warmup = 3 if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -232,6 +232,40 @@ int og_pm_longrange(og_pm *pm, const float *pos, const float *mass, uint64_t n, 
                     uint64_t n_active, float *acc_out, float *pot_out, og_stream stream);
 void og_pm_free(og_pm *pm, og_stream stream);
 
+/* ---- row f2: the time-step shell around the force calls --------------------------------- */
+
+/*
+ * PAPER.md:80 (time bins with few active particles), :82 (all particles are drifted at the onset of a GPU step),
+ * :320 (find_sync_point_and_drift).  Gadget-2's individual power-of-two time steps (readings R37..R42, DESIGN.md
+ * Sec. 11): one tick = dt_max / 2^bmax; a particle in bin b (u8, 0..bmax) has a step of 2^(bmax - b) ticks and is
+ * active at the ticks its step divides.  One step of a host loop is
+ *     og_ts_next_tick -> og_ts_drift (all particles, dt = (next - tick) dt_max / 2^bmax) -> og_ts_active_list ->
+ *     og_tree_build + og_shortrange_accel (active_idx, a_old gathered by the caller) [+ og_pm_longrange] -> og_ts_kick.
+ * All array pointers DEVICE; state arrays (pos, vel, bin, a_old) are caller-owned and updated in place.
+ *
+ * og_ts_drift       pos f32 [n][3] += vel f32 [n][3] * dt, wrapped into [0, box).  Enqueues.
+ * og_ts_next_tick   *next_tick_host (HOST) = the next tick > `tick` at which some particle is active (`tick` must be a
+ *                   synchronisation point, 0 at the start).  Synchronises `stream`.
+ * og_ts_active_list active_idx u32 [>= n] receives, ascending, the particles active at `tick`; *n_active_host (HOST)
+ *                   their number.  Synchronises `stream` (the host sizes the force call with it).
+ * og_ts_kick        for the active particles (active_idx NULL -> all n in identity order), with acc f32 [n_active][3]
+ *                   in active order and soft f32 [n] (eps): |a| in fp32; wanted bin = smallest b with
+ *                   4^b >= dt_max^2 |a| / (2 eta eps) (fp32, fixed operation order); the step shrinks freely and grows
+ *                   by one level only at a tick the larger step divides; vel += acc (dt_old + dt_new) / 2 (first != 0:
+ *                   start of the integration, wanted bin taken as is, opening half kick dt_new / 2 only); bin and
+ *                   a_old f32 [n] (= |a|, the next walk's opening-criterion input) updated.  Enqueues.
+ * scratch: DEVICE, og_ts_scratch_bytes(n) bytes.  bmax <= 40.
+ */
+size_t og_ts_scratch_bytes(uint64_t n);
+int og_ts_drift(float *pos, const float *vel, uint64_t n, float dt, float box, og_stream stream);
+int og_ts_next_tick(const uint8_t *bin, uint64_t n, uint64_t tick, uint32_t bmax, uint64_t *next_tick_host,
+                    void *scratch, size_t scratch_bytes, og_stream stream);
+int og_ts_active_list(const uint8_t *bin, uint64_t n, uint64_t tick, uint32_t bmax, uint32_t *active_idx,
+                      uint64_t *n_active_host, void *scratch, size_t scratch_bytes, og_stream stream);
+int og_ts_kick(float *vel, uint8_t *bin, float *a_old, const uint32_t *active_idx, uint64_t n, uint64_t n_active,
+               const float *acc, const float *soft, float eta, float dt_max, uint32_t bmax, uint64_t tick, int first,
+               og_stream stream);
+
 /* Returns the device memory that freed trees / finished calls left cached in the library's
  * stream-ordered pool of the current device to the driver (the pool keeps arenas for reuse by
  * the next og_tree_build; a host code that needs the memory for something else calls this).

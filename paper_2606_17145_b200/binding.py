@@ -111,6 +111,16 @@ def _load():
     lib.og_pm_longrange.argtypes = [vp, vp, vp, u64, u32p, u64, vp, vp, vp]
     lib.og_pm_free.restype = None
     lib.og_pm_free.argtypes = [vp, vp]
+    lib.og_ts_scratch_bytes.restype = C.c_size_t
+    lib.og_ts_scratch_bytes.argtypes = [u64]
+    lib.og_ts_drift.restype = C.c_int
+    lib.og_ts_drift.argtypes = [vp, vp, u64, C.c_float, C.c_float, vp]
+    lib.og_ts_next_tick.restype = C.c_int
+    lib.og_ts_next_tick.argtypes = [vp, u64, u64, C.c_uint32, C.POINTER(u64), vp, C.c_size_t, vp]
+    lib.og_ts_active_list.restype = C.c_int
+    lib.og_ts_active_list.argtypes = [vp, u64, u64, C.c_uint32, vp, C.POINTER(u64), vp, C.c_size_t, vp]
+    lib.og_ts_kick.restype = C.c_int
+    lib.og_ts_kick.argtypes = [vp, vp, vp, u32p, u64, u64, vp, vp, C.c_float, C.c_float, C.c_uint32, u64, C.c_int, vp]
     return lib
 
 
@@ -119,7 +129,7 @@ _lib = _load()
 EXPORTS = ("og_tree_workspace_bytes", "og_tree_build", "og_shortrange_accel", "og_tree_get", "og_tree_status",
            "og_tree_stats", "og_tree_free", "og_last_error", "og_morton_keys", "og_radix_sort_scratch_bytes",
            "og_radix_sort_pairs", "og_shortrange_accel_host", "og_trim", "og_pm_create", "og_pm_longrange",
-           "og_pm_free")
+           "og_pm_free", "og_ts_scratch_bytes", "og_ts_drift", "og_ts_next_tick", "og_ts_active_list", "og_ts_kick")
 
 
 def _err() -> str:
@@ -343,3 +353,39 @@ def og_pm_free(pm: Pm, stream=None):
     if pm.handle:
         h, pm.handle = pm.handle, 0
         _lib.og_pm_free(h, _stream(stream) if torch.cuda.is_available() else None)
+
+
+# ---- row f2: time-step shell ---------------------------------------------------------------------------------
+def og_ts_scratch_bytes(n: int) -> int:
+    return int(_lib.og_ts_scratch_bytes(n))
+
+
+def og_ts_drift(pos: torch.Tensor, vel: torch.Tensor, dt: float, box: float, stream=None):
+    _check(_lib.og_ts_drift(_dev(pos, torch.float32, "pos"), _dev(vel, torch.float32, "vel"), int(pos.shape[0]), float(dt),
+                            float(box), _stream(stream)))
+
+
+def og_ts_next_tick(bins: torch.Tensor, tick: int, bmax: int, scratch: torch.Tensor, stream=None) -> int:
+    out = C.c_uint64(0)
+    _check(_lib.og_ts_next_tick(_dev(bins, torch.uint8, "bin"), int(bins.shape[0]), int(tick), int(bmax), C.byref(out),
+                                scratch.data_ptr(), scratch.numel() * scratch.element_size(), _stream(stream)))
+    return int(out.value)
+
+
+def og_ts_active_list(bins: torch.Tensor, tick: int, bmax: int, active_idx: torch.Tensor, scratch: torch.Tensor,
+                      stream=None) -> int:
+    """Fills active_idx (int32 CUDA tensor of >= n elements) with the ascending active particles; -> their number."""
+    out = C.c_uint64(0)
+    _check(_lib.og_ts_active_list(_dev(bins, torch.uint8, "bin"), int(bins.shape[0]), int(tick), int(bmax),
+                                  _dev(active_idx, torch.int32, "active_idx"), C.byref(out), scratch.data_ptr(),
+                                  scratch.numel() * scratch.element_size(), _stream(stream)))
+    return int(out.value)
+
+
+def og_ts_kick(vel: torch.Tensor, bins: torch.Tensor, a_old: torch.Tensor, active_idx: torch.Tensor | None, n_active: int,
+               acc: torch.Tensor, soft: torch.Tensor, eta: float, dt_max: float, bmax: int, tick: int, first: bool,
+               stream=None):
+    _check(_lib.og_ts_kick(_dev(vel, torch.float32, "vel"), _dev(bins, torch.uint8, "bin"), _dev(a_old, torch.float32, "a_old"),
+                           None if active_idx is None else _dev(active_idx, torch.int32, "active_idx"), int(vel.shape[0]),
+                           int(n_active), _dev(acc, torch.float32, "acc"), _dev(soft, torch.float32, "soft"), float(eta),
+                           float(dt_max), int(bmax), int(tick), 1 if first else 0, _stream(stream)))
