@@ -537,6 +537,65 @@ def run_timesteps(args):
     return 0
 
 
+def run_sph(args):
+    """--sph N_DES (row f3): og_sph_density on the workload's particles (all of them targets), timed
+    twice: cold (starting radius from the tree) and warm (h_guess = the previous answer, the regime of a running
+    simulation).  Prints its own JSON line with the oracle (oracle/sph.py) timed on a bounded sample beside it."""
+    import torch
+    from paper_2606_17145_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    w = W.make(args.workload)
+    n_des = float(args.sph)
+    prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8)
+    pos, mass, eps = (torch.from_numpy(x).to(dev) for x in (w.pos, w.mass, w.eps))
+    tree = B.og_tree_build(pos, mass, eps, w.L, prm)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def timed(guess):
+        for _ in range(max(args.warmup, 1)):
+            h, rho, nn = B.og_sph_density(tree, n_des, h_guess=guess)
+        torch.cuda.synchronize()
+        e0, e1 = ev(), ev()
+        e0.record()
+        for _ in range(args.steps):
+            h, rho, nn = B.og_sph_density(tree, n_des, h_guess=guess)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps, h, rho, nn
+
+    ms_cold, h, rho, nn = timed(None)
+    ms_warm, h2, _, _ = timed(h.clone())
+    status = B.og_tree_status(tree)
+    line = {"mode": "sph_density", "metric": "SPH density + smoothing-length targets/s (neighbour walk + root of N(h) = n_des) on B200",
+            "value": w.n / (ms_cold * 1e-3), "unit": "particles/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_cold, "ms_per_step_with_h_guess": ms_warm, "value_with_h_guess": w.n / (ms_warm * 1e-3),
+            "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "n": w.n, "n_des": n_des, "tol_n": 0.0, "box": w.L},
+            "checks": {"mean_N": float(nn.mean().item()), "max_abs_N_minus_n_des": float((nn - n_des).abs().max().item()),
+                       "max_rel_h_warm_vs_cold": float(((h2 - h).abs() / h).max().item()), "mean_h": float(h.mean().item())},
+            "status": status}
+    if not args.no_cpu_baseline:
+        import time
+        from oracle import sph as osph
+        rng = np.random.default_rng(4242)
+        t = np.sort(rng.choice(w.n, size=args.sph_cpu_sample, replace=False))
+        p64, m64 = w.pos.astype(np.float64), w.mass.astype(np.float64)
+        t0 = time.perf_counter()
+        ho, ro, no = osph.sph_density(p64, m64, w.L, n_des, targets=t)
+        dt = time.perf_counter() - t0
+        hg = h.cpu().numpy().astype(np.float64)[t]
+        line["cpu_baseline"] = {"value": len(t) / dt, "unit": "particles/s", "cores": 1, "kind": "oracle",
+                                "sample": f"oracle/sph.py on {len(t)} seeded random targets of the same workload (cKDTree build "
+                                          f"included, {dt:.1f} s, 1 thread)",
+                                "max_rel_h_vs_oracle_on_sample": float((np.abs(hg - ho) / ho).max())}
+    B.og_tree_free(tree)
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -552,9 +611,14 @@ def main():
                          "a Morton range of the active targets (SURVEY.md Sec. 8.5)")
     ap.add_argument("--timesteps", type=int, default=0,
                     help="row f2: run this many synchronisation steps of the time-step shell instead of the standard step")
+    ap.add_argument("--sph", type=float, default=0.0,
+                    help="row f3: time og_sph_density with this desired neighbour number instead of the standard step")
+    ap.add_argument("--sph-cpu-sample", type=int, default=300)
     args = ap.parse_args()
     if args.timesteps > 0:
         return run_timesteps(args)
+    if args.sph > 0:
+        return run_sph(args)
     if args.warmup < 3:
         args.warmup = 3 if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -51,7 +51,8 @@ typedef enum {
     OG_ERR_NODE_OVERFLOW = -3,   /* canonical octree needs more than max_nodes nodes (R6)  */
     OG_ERR_CUDA = -4,
     OG_ERR_BAD_POSITION = -5,    /* OG_VALIDATE_POS: some x not in [0, box)                */
-    OG_ERR_STACK_OVERFLOW = -6   /* walk traversal stack exceeded its spill capacity       */
+    OG_ERR_STACK_OVERFLOW = -6,  /* walk traversal stack exceeded its spill capacity       */
+    OG_ERR_NGB_OVERFLOW = -7     /* og_sph_density: no root / neighbour stack exceeded      */
 } og_status;
 
 /* og_params.flags */
@@ -265,6 +266,32 @@ int og_ts_active_list(const uint8_t *bin, uint64_t n, uint64_t tick, uint32_t bm
 int og_ts_kick(float *vel, uint8_t *bin, float *a_old, const uint32_t *active_idx, uint64_t n, uint64_t n_active,
                const float *acc, const float *soft, float eta, float dt_max, uint32_t bmax, uint64_t tick, int first,
                og_stream stream);
+
+/* ---- row f3: SPH density / smoothing length on the same tree -------------------------------- */
+
+/*
+ * PAPER.md:61 ("the SPH density module ... operates as an iterative process, aiming to determine a smoothing length
+ * containing a fixed number of neighbours"), :74 ("collects all neighbours within a sphere around the target
+ * particle").  Readings R43..R47 (Gadget-2's SPH): cubic-spline kernel with compact
+ * support h, W(r, h) = (8 / (pi h^3)) w(r / h); kernel-weighted neighbour number N_i(h) = (4 pi / 3) h^3 sum_j
+ * W(r_ij, h) over ALL particles of the tree (j = i included, nearest periodic image); h_i = the root of
+ * N_i(h) = n_des; rho_i = sum_j m_j W(r_ij, h_i).  The root is found per target on the neighbours collected by a
+ * walk of the tree; the iteration stops at |N - n_des| <= tol_n or at fp32 resolution of h (tol_n = 0: always the
+ * latter).  fp32 arithmetic, fixed summation order (bit-reproducible run to run).
+ *   tree       a tree from og_tree_build (its particles are the SPH particles; masses from the tree)
+ *   active_idx DEVICE u32 [n_active] ORIGINAL indices of the targets, or NULL -> all n in identity order
+ *   n_des      32/3 < n_des <= 256 (N(h) -> 32/3 as h -> 0 for an isolated particle)
+ *   h_guess    DEVICE f32 [n_active] starting radius per target in active order (e.g. the previous step's h), or
+ *              NULL -> derived from the tree (half the side of the deepest ancestor cell holding n_des particles)
+ *   h_out      DEVICE f32 [n_active]; rho_out, nn_out (N at the returned h): DEVICE f32 [n_active] or NULL
+ * Enqueues on `stream` (ordered after the tree's build).  Neighbour candidates are kept in a per-warp list of 1024
+ * entries; a target whose root sphere holds more (a void particle whose kernel rim grazes a dense clump) is solved
+ * by re-walking the tree for every trial h instead (same result, slower).  A target with more than 3 n_des / 32
+ * coincident particles (N(h) > n_des for every h: no root), or whose pending nodes exceed even the fallback's stack,
+ * latches OG_ERR_NGB_OVERFLOW (og_tree_status) and gets h = rho = N = 0.
+ */
+int og_sph_density(const og_tree *tree, const uint32_t *active_idx, uint64_t n_active, float n_des, float tol_n,
+                   const float *h_guess, float *h_out, float *rho_out, float *nn_out, og_stream stream);
 
 /* Returns the device memory that freed trees / finished calls left cached in the library's
  * stream-ordered pool of the current device to the driver (the pool keeps arenas for reuse by

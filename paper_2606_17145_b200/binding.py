@@ -23,6 +23,7 @@ OG_ERR_NODE_OVERFLOW = -3
 OG_ERR_CUDA = -4
 OG_ERR_BAD_POSITION = -5
 OG_ERR_STACK_OVERFLOW = -6
+OG_ERR_NGB_OVERFLOW = -7
 # flags
 OG_PERIODIC = 1
 OG_VALIDATE_POS = 2
@@ -119,6 +120,8 @@ def _load():
     lib.og_ts_next_tick.argtypes = [vp, u64, u64, C.c_uint32, C.POINTER(u64), vp, C.c_size_t, vp]
     lib.og_ts_active_list.restype = C.c_int
     lib.og_ts_active_list.argtypes = [vp, u64, u64, C.c_uint32, vp, C.POINTER(u64), vp, C.c_size_t, vp]
+    lib.og_sph_density.restype = C.c_int
+    lib.og_sph_density.argtypes = [vp, u32p, u64, C.c_float, C.c_float, vp, vp, vp, vp, vp]
     lib.og_ts_kick.restype = C.c_int
     lib.og_ts_kick.argtypes = [vp, vp, vp, u32p, u64, u64, vp, vp, C.c_float, C.c_float, C.c_uint32, u64, C.c_int, vp]
     return lib
@@ -129,7 +132,8 @@ _lib = _load()
 EXPORTS = ("og_tree_workspace_bytes", "og_tree_build", "og_shortrange_accel", "og_tree_get", "og_tree_status",
            "og_tree_stats", "og_tree_free", "og_last_error", "og_morton_keys", "og_radix_sort_scratch_bytes",
            "og_radix_sort_pairs", "og_shortrange_accel_host", "og_trim", "og_pm_create", "og_pm_longrange",
-           "og_pm_free", "og_ts_scratch_bytes", "og_ts_drift", "og_ts_next_tick", "og_ts_active_list", "og_ts_kick")
+           "og_pm_free", "og_ts_scratch_bytes", "og_ts_drift", "og_ts_next_tick", "og_ts_active_list", "og_ts_kick",
+           "og_sph_density")
 
 
 def _err() -> str:
@@ -389,3 +393,18 @@ def og_ts_kick(vel: torch.Tensor, bins: torch.Tensor, a_old: torch.Tensor, activ
                            None if active_idx is None else _dev(active_idx, torch.int32, "active_idx"), int(vel.shape[0]),
                            int(n_active), _dev(acc, torch.float32, "acc"), _dev(soft, torch.float32, "soft"), float(eta),
                            float(dt_max), int(bmax), int(tick), 1 if first else 0, _stream(stream)))
+
+
+def og_sph_density(tree: Tree, n_des: float, active_idx: torch.Tensor | None = None, h_guess: torch.Tensor | None = None,
+                   tol_n: float = 0.0, want_rho: bool = True, want_nn: bool = True, stream=None):
+    """Row f3.  -> (h [na], rho [na] | None, N [na] | None) in the caller's order."""
+    na = tree.n if active_idx is None else int(active_idx.shape[0])
+    dev = torch.device("cuda", torch.cuda.current_device())
+    h = torch.empty(na, dtype=torch.float32, device=dev)
+    rho = torch.empty(na, dtype=torch.float32, device=dev) if want_rho else None
+    nn = torch.empty(na, dtype=torch.float32, device=dev) if want_nn else None
+    _check(_lib.og_sph_density(tree.handle, None if active_idx is None else _dev(active_idx, torch.int32, "active_idx"), na,
+                               float(n_des), float(tol_n), _dev(h_guess, torch.float32, "h_guess"),
+                               _dev(h, torch.float32, "h_out"), _dev(rho, torch.float32, "rho_out"),
+                               _dev(nn, torch.float32, "nn_out"), _stream(stream)))
+    return h, rho, nn

@@ -144,6 +144,7 @@ int status_from_bits(uint32_t bits)
     if (bits & OG_DEV_BAD_POSITION) return OG_ERR_BAD_POSITION;
     if (bits & OG_DEV_STACK_OVERFLOW) return OG_ERR_STACK_OVERFLOW;
     if (bits & OG_DEV_BAD_INDEX) return OG_ERR_INVALID_ARG;
+    if (bits & OG_DEV_NGB_OVERFLOW) return OG_ERR_NGB_OVERFLOW;
     return OG_OK;
 }
 
@@ -320,6 +321,34 @@ extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx,
     t->walked = true;
     OG_ACC_TRY(cudaFreeAsync(tmp, st));
 #undef OG_ACC_TRY
+    return OG_OK;
+}
+
+extern "C" int og_sph_density(const og_tree *t, const uint32_t *active_idx, uint64_t n_active, float n_des, float tol_n,
+                              const float *h_guess, float *h_out, float *rho_out, float *nn_out, og_stream stream)
+{
+    g_err[0] = 0;
+    if (!t) { og_set_error("tree is NULL"); return OG_ERR_INVALID_ARG; }
+    if (n_active == 0) return OG_OK;
+    if (!h_out) { og_set_error("h_out is NULL"); return OG_ERR_INVALID_ARG; }
+    if (!active_idx && n_active != t->n) {
+        og_set_error("active_idx == NULL requires n_active == n (%llu != %llu)", (unsigned long long)n_active,
+                     (unsigned long long)t->n);
+        return OG_ERR_INVALID_ARG;
+    }
+    if (n_active >= (1ull << 31)) { og_set_error("n_active out of range"); return OG_ERR_INVALID_ARG; }
+    if (!(n_des > 32.0f / 3.0f) || !(n_des <= 256.0f) || !(tol_n >= 0.0f)) {
+        og_set_error("og_sph_density needs 32/3 < n_des <= 256 and tol_n >= 0 (n_des = %g, tol_n = %g)", n_des, tol_n);
+        return OG_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (st != t->build_stream) OG_CUDA_TRY(cudaStreamWaitEvent(st, t->ev_built, 0), return OG_ERR_CUDA);
+    OG_CUDA_TRY(ogk_sph_density(t, active_idx, n_active, n_des, tol_n, h_guess, h_out, rho_out, nn_out, st),
+                return OG_ERR_CUDA);
+    // og_tree_free and og_tree_status wait for this call like for a walk
+    if (t->walked) OG_CUDA_TRY(cudaStreamWaitEvent(st, t->ev_walked, 0), return OG_ERR_CUDA);
+    OG_CUDA_TRY(cudaEventRecord(t->ev_walked, st), return OG_ERR_CUDA);
+    t->walked = true;
     return OG_OK;
 }
 

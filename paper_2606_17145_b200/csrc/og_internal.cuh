@@ -13,6 +13,7 @@
 #define OG_DEV_BAD_POSITION 2u
 #define OG_DEV_STACK_OVERFLOW 4u
 #define OG_DEV_BAD_INDEX 8u
+#define OG_DEV_NGB_OVERFLOW 16u   // og_sph_density: the neighbour candidates of a target do not fit its list
 
 // Counter slots (og_tree::d_counters), see og_stats.
 enum { OGC_V_FULL = 0, OGC_V_CULL, OGC_A_IN, OGC_P_IN, OGC_P_SOFT, OGC_P_OUT, OGC_FP64,
@@ -119,6 +120,9 @@ cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t 
                      cudaStream_t st);
 size_t ogk_walk_spill_bytes(int sm_count, uint32_t spill_entries);
 uint32_t ogk_walk_spill_entries(const og_params *p);
+// f3
+cudaError_t ogk_sph_density(const og_tree *t, const uint32_t *active_idx, uint64_t n_active, float n_des, float tol_n,
+                            const float *h_guess, float *h_out, float *rho_out, float *nn_out, cudaStream_t st);
 // helpers for the active subset
 cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_perm, uint64_t n,
                              uint64_t n_active, uint64_t *keys, uint32_t *vals, uint32_t *d_status,

@@ -1,0 +1,341 @@
+// sph.cu -- row f3 of SURVEY.md Sec. 8: SPH density / smoothing length on the gravity tree.
+// PAPER.md:61 ("the SPH density module ... operates as an iterative process, aiming to determine a smoothing
+// length containing a fixed number of neighbours"), :74 ("collects all neighbours within a sphere around the
+// target particle and processes them in a separate evaluate function").  Readings R43..R47, DESIGN.md Sec. 12.
+//
+// k_sph_density: one warp per target.
+//   1. radius H: the caller's h_guess, or the half side of the deepest ancestor of the target that still holds
+//      n_des particles (found by descending the target's own path from the root);
+//   2. COLLECT: the warp walks the tree (32 nodes per step from a warp-private stack in shared memory; a node is
+//      opened when the nearest image of its tight AABB is within H of the target; children are contiguous) and
+//      appends (r, m) of every particle with r < H to a candidate list in shared memory (ballot compaction);
+//   3. N(H) < n_des: H *= 2^(1/3), back to 2.  The list does not fit: H *= 0.8, back to 2, from then on growing by
+//      1.04 only (if the list overflows again before N(H) reaches n_des, OG_DEV_NGB_OVERFLOW is latched);
+//   4. ROOT: N(h) = n_des on the list (every h <= H sees all its neighbours there): Newton steps kept inside a
+//      bisection bracket, N and dN/dh summed by the lanes over their slices and reduced by shuffles (fixed order:
+//      bit-reproducible); stops at |N - n_des| <= tol_n or when the bracket has collapsed to fp32 resolution;
+//   5. rho = (8 / (pi h^3)) sum m w(r / h) with that h.
+#include "og_internal.cuh"
+
+namespace {
+
+constexpr int SPH_WARPS = 4;
+constexpr int SPH_CAP = 1024;    // candidates per warp
+constexpr int SPH_QCAP = 512;    // pending nodes per warp
+
+struct __align__(16) SphSmem {
+    float cr[SPH_CAP];           // distance to the target
+    float cm[SPH_CAP];           // mass
+    uint32_t q[SPH_QCAP];
+};
+
+struct SphArgs {
+    const float4 *lo, *hi;
+    const uint2 *info;
+    const uint32_t *node_first, *node_count, *first_child;
+    const uint8_t *nchild;
+    const float4 *spos;
+    const uint32_t *inv_perm, *perm;
+    const uint32_t *active_idx;  // NULL: target k = sorted slot k, written at perm[k]
+    const float *h_guess;        // NULL or [n_active] in the caller's order
+    float *h_out, *rho_out, *nn_out;
+    uint32_t n, n_active;
+    float L, invL, n_des, tol_n;
+    uint32_t *status;
+};
+
+__device__ __forceinline__ float sph_wrap(float d, float L, float invL) { return fmaf(-L, rintf(d * invL), d); }
+
+// R43: w(u) and u w'(u) of the cubic spline with support u <= 1
+__device__ __forceinline__ void sph_w(float u, float &w, float &uwp)
+{
+    if (u <= 0.5f) {
+        w = fmaf(u * u, fmaf(6.0f, u, -6.0f), 1.0f);
+        uwp = u * u * fmaf(18.0f, u, -12.0f);
+    } else if (u <= 1.0f) {
+        const float v = 1.0f - u;
+        w = 2.0f * v * v * v;
+        uwp = -6.0f * v * v * u;
+    } else {
+        w = 0.0f; uwp = 0.0f;
+    }
+}
+
+__device__ __forceinline__ float warp_sum(float v)
+{
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// N(h) and h dN/dh over the candidate list (R44): every lane returns the same bits
+__device__ __forceinline__ void sph_number(const SphSmem &s, int cnt, float h, uint32_t lane, float &N, float &hdN)
+{
+    const float hinv = 1.0f / h;
+    float a = 0.0f, b = 0.0f;
+    for (int j = lane; j < cnt; j += 32) {
+        float w, uwp;
+        sph_w(s.cr[j] * hinv, w, uwp);
+        a += w; b += uwp;
+    }
+    const float k = 32.0f / 3.0f;
+    N = k * warp_sum(a);
+    hdN = -k * warp_sum(b);    // dN/dh = -(32/3) sum w'(u) u / h
+}
+
+// Step 2.  STORE: fills the candidate list with every particle closer than H to (px, py, pz) and returns their number,
+// or -1 if the list or the node stack overflowed.  !STORE (the fallback of a target whose candidates do not fit the
+// list): nothing is stored, the lanes add w, u w' and m w of the particles inside H = h to (sa, sb, sc) on the fly, and
+// the node stack may use the whole per-warp area; -1 only if even that stack overflows.
+template <bool STORE>
+__device__ int sph_scan(const SphArgs &a, SphSmem &s, float px, float py, float pz, float H, uint32_t lane, float &sa,
+                        float &sb, float &sc)
+{
+    const float H2 = H * H;
+    const float H2n = H2 * (1.0f + 1.0e-5f);      // nodes: conservative
+    const float pad = 4.0e-7f * a.L;              // rounding of the box centre / half size
+    const float hinv = 1.0f / H;
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t *q = STORE ? s.q : reinterpret_cast<uint32_t *>(&s);
+    const int qcap = STORE ? SPH_QCAP : (int)(sizeof(SphSmem) / sizeof(uint32_t));
+    int qn = 1, cnt = 0;
+    if (lane == 0) q[0] = 0u;
+    __syncwarp();
+    while (qn > 0) {
+        const int take = min(qn, 32);
+        qn -= take;
+        bool hit = false;
+        uint2 info = make_uint2(0u, 0u);
+        if ((int)lane < take) {
+            const uint32_t node = q[qn + lane];
+            const float4 lo = __ldg(a.lo + node), hi = __ldg(a.hi + node);
+            info = __ldg(a.info + node);
+            const float dx = fmaxf(fabsf(sph_wrap(0.5f * (lo.x + hi.x) - px, a.L, a.invL)) - (0.5f * (hi.x - lo.x) + pad), 0.0f);
+            const float dy = fmaxf(fabsf(sph_wrap(0.5f * (lo.y + hi.y) - py, a.L, a.invL)) - (0.5f * (hi.y - lo.y) + pad), 0.0f);
+            const float dz = fmaxf(fabsf(sph_wrap(0.5f * (lo.z + hi.z) - pz, a.L, a.invL)) - (0.5f * (hi.z - lo.z) + pad), 0.0f);
+            hit = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) <= H2n;
+        }
+        __syncwarp();
+        const bool leaf = (info.y & OG_LEAF_BIT) != 0u;
+        const uint32_t c = info.y & ~OG_LEAF_BIT;
+        const uint32_t nch = (hit && !leaf) ? c : 0u;
+        uint32_t incl = nch;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= (uint32_t)o) incl += y;
+        }
+        const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
+        if (qn + (int)total > qcap) return -1;
+        for (uint32_t k = 0; k < nch; ++k) q[qn + (incl - nch) + k] = info.x + k;
+        qn += (int)total;
+        uint32_t lb = __ballot_sync(0xffffffffu, hit && leaf);
+        while (lb) {
+            const int src = __ffs(lb) - 1;
+            lb &= lb - 1u;
+            const uint32_t first = __shfl_sync(0xffffffffu, info.x, src);
+            const uint32_t pc = __shfl_sync(0xffffffffu, c, src);
+            for (uint32_t base = 0; base < pc; base += 32u) {
+                bool in = false;
+                float r2 = 0.0f, m = 0.0f;
+                if (base + lane < pc) {
+                    const float4 pq = __ldg(a.spos + first + base + lane);
+                    const float dx = sph_wrap(pq.x - px, a.L, a.invL), dy = sph_wrap(pq.y - py, a.L, a.invL),
+                                dz = sph_wrap(pq.z - pz, a.L, a.invL);
+                    r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    in = r2 < H2;
+                    m = pq.w;
+                }
+                const uint32_t b = __ballot_sync(0xffffffffu, in);
+                const int nb = __popc(b);
+                if (STORE) {
+                    if (cnt + nb > SPH_CAP) return -1;
+                    if (in) {
+                        const int p = cnt + __popc(b & lt);
+                        s.cr[p] = sqrtf(r2);
+                        s.cm[p] = m;
+                    }
+                } else if (in) {
+                    float w, uwp;
+                    sph_w(sqrtf(r2) * hinv, w, uwp);
+                    sa += w; sb += uwp; sc = fmaf(m, w, sc);
+                }
+                cnt += nb;
+            }
+        }
+        __syncwarp();
+    }
+    return cnt;
+}
+
+// The fallback evaluator: N(h), h dN/dh and sum m w by a walk of the tree with radius h.  false: stack overflow.
+__device__ __forceinline__ bool sph_number_stream(const SphArgs &a, SphSmem &s, float px, float py, float pz, float h,
+                                                  uint32_t lane, float &N, float &hdN, float &msum)
+{
+    float sa = 0.0f, sb = 0.0f, sc = 0.0f;
+    const int cnt = sph_scan<false>(a, s, px, py, pz, h, lane, sa, sb, sc);
+    __syncwarp();
+    const float k = 32.0f / 3.0f;
+    N = k * warp_sum(sa); hdN = -k * warp_sum(sb); msum = warp_sum(sc);
+    return cnt >= 0;
+}
+
+__global__ void __launch_bounds__(SPH_WARPS * 32) k_sph_density(const __grid_constant__ SphArgs a)
+{
+    __shared__ SphSmem sm[SPH_WARPS];
+    const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
+    SphSmem &s = sm[wid];
+    const uint32_t nwarps = gridDim.x * SPH_WARPS;
+    for (uint32_t k = blockIdx.x * SPH_WARPS + wid; k < a.n_active; k += nwarps) {
+        uint32_t slot, out;
+        if (a.active_idx) {
+            const uint32_t i = __ldg(a.active_idx + k);
+            if (i >= a.n) { if (lane == 0) atomicOr(a.status, OG_DEV_BAD_INDEX); continue; }
+            slot = __ldg(a.inv_perm + i); out = k;
+        } else {
+            slot = k; out = __ldg(a.perm + k);
+        }
+        const float4 p = __ldg(a.spos + slot);
+        float H;
+        if (a.h_guess) {
+            H = __ldg(a.h_guess + out);
+            if (!(H > 0.0f)) H = 1.0e-3f * a.L;
+        } else {
+            // deepest ancestor of the target with at least n_des particles (the root if there is none)
+            uint32_t node = 0u, level = 0u;
+            for (;;) {
+                const uint32_t nc = __ldg(a.nchild + node);
+                if (nc == 0u) break;
+                const uint32_t fc = __ldg(a.first_child + node);
+                uint32_t cf = 0xffffffffu, cc = 0u;
+                if (lane < nc) { cf = __ldg(a.node_first + fc + lane); cc = __ldg(a.node_count + fc + lane); }
+                const uint32_t mine = __ballot_sync(0xffffffffu, lane < nc && slot >= cf && slot < cf + cc);
+                if (mine == 0u) break;
+                const int src = __ffs(mine) - 1;
+                const uint32_t ccnt = __shfl_sync(0xffffffffu, cc, src);
+                if ((float)ccnt < a.n_des) break;
+                node = fc + (uint32_t)src; ++level;
+            }
+            H = 0.5f * a.L * __uint_as_float((127u - level) << 23);
+        }
+        const float hcap = 0.5f * a.L * (1.0f - 1.0e-6f);
+        H = fminf(H, hcap);
+        // steps 2, 3: a sphere that holds the root of N(h) = n_des and fits the list
+        int cnt = 0;
+        float NH = 0.0f, hdN = 0.0f;
+        bool shrunk = false, regrown = false, fail = false;   // fail: pending nodes exceed even the fallback's stack
+        float grow = 1.2599211f;
+        for (int tries = 0; tries < 200; ++tries) {
+            { float d0 = 0.f, d1 = 0.f, d2 = 0.f; cnt = sph_scan<true>(a, s, p.x, p.y, p.z, H, lane, d0, d1, d2); }
+            __syncwarp();
+            if (cnt < 0) {
+                if (regrown) break;            // no sphere both holds n_des and fits the list
+                H *= 0.8f; shrunk = true; grow = 1.04f;
+                continue;
+            }
+            sph_number(s, cnt, H, lane, NH, hdN);
+            if (NH >= a.n_des || H >= hcap) break;
+            regrown = shrunk;
+            H = fminf(H * grow, hcap);
+        }
+        if (cnt < 0) {
+            // the candidates of the sphere that holds the root do not fit the list (a target in a void next to a dense
+            // clump: thousands of neighbours near the rim of its kernel): the same root search with every N(h) summed
+            // by a walk of the tree
+            float lo = 0.0f, hi = 0.0f, h = H, N = 0.0f, msum = 0.0f;      // hi = 0: no upper bound yet
+            for (int it = 0; it < 400; ++it) {
+                if (!sph_number_stream(a, s, p.x, p.y, p.z, h, lane, N, hdN, msum)) { fail = true; break; }
+                if (fabsf(N - a.n_des) <= a.tol_n) break;
+                if (N > a.n_des) hi = h; else lo = h;
+                if (lo == 0.0f && hi != 0.0f && hi < 1.0e-12f * a.L) { fail = true; break; }   // no root: coincident pile
+                float hn;
+                if (hi == 0.0f) {
+                    if (h >= hcap) break;
+                    hn = fminf(h * 1.2599211f, hcap);
+                } else {
+                    if (hi - lo <= 2.4e-7f * hi) break;
+                    hn = (hdN > 0.0f) ? h * (1.0f - (N - a.n_des) / hdN) : 0.0f;
+                    if (!(hn > lo && hn < hi)) hn = 0.5f * (lo + hi);
+                    if (hn == h) break;
+                }
+                h = hn;
+            }
+            if (lane == 0) {
+                if (fail) { atomicOr(a.status, OG_DEV_NGB_OVERFLOW); h = 0.0f; N = 0.0f; msum = 0.0f; }
+                const float hinv = fail ? 0.0f : 1.0f / h;
+                a.h_out[out] = h;
+                if (a.rho_out) a.rho_out[out] = 2.5464790894703255f * hinv * hinv * hinv * msum;
+                if (a.nn_out) a.nn_out[out] = N;
+            }
+            __syncwarp();
+            continue;
+        }
+        // step 4: root of N(h) = n_des in (0, H]; N is increasing in h
+        float lo = 0.0f, hi = H, h = H, N = NH;
+        bool noroot = false;       // more than 3 n_des / 32 particles coincide with the target: N(h) > n_des for every h
+        if (NH >= a.n_des) {
+            for (int it = 0; it < 100; ++it) {
+                if (fabsf(N - a.n_des) <= a.tol_n) break;
+                if (N > a.n_des) hi = h; else lo = h;
+                if (lo == 0.0f && hi < 1.0e-12f * a.L) { noroot = true; break; }
+                if (hi - lo <= 2.4e-7f * hi) break;
+                float hn = (hdN > 0.0f) ? h * (1.0f - (N - a.n_des) / hdN) : 0.0f;     // Newton step
+                if (!(hn > lo && hn < hi)) hn = 0.5f * (lo + hi);
+                if (hn == h) break;
+                h = hn;
+                sph_number(s, cnt, h, lane, N, hdN);
+            }
+        }
+        if (noroot) {
+            if (lane == 0) {
+                atomicOr(a.status, OG_DEV_NGB_OVERFLOW);
+                a.h_out[out] = 0.0f;
+                if (a.rho_out) a.rho_out[out] = 0.0f;
+                if (a.nn_out) a.nn_out[out] = 0.0f;
+            }
+            __syncwarp();
+            continue;
+        }
+        // step 5
+        const float hinv = 1.0f / h;
+        float sum = 0.0f;
+        for (int j = lane; j < cnt; j += 32) {
+            float w, uwp;
+            sph_w(s.cr[j] * hinv, w, uwp);
+            sum = fmaf(s.cm[j], w, sum);
+        }
+        sum = warp_sum(sum);
+        if (lane == 0) {
+            a.h_out[out] = h;
+            if (a.rho_out) a.rho_out[out] = 2.5464790894703255f * hinv * hinv * hinv * sum;   // 8 / pi
+            if (a.nn_out) a.nn_out[out] = N;
+        }
+        __syncwarp();
+    }
+}
+
+}  // namespace
+
+cudaError_t ogk_sph_density(const og_tree *t, const uint32_t *active_idx, uint64_t n_active, float n_des, float tol_n,
+                            const float *h_guess, float *h_out, float *rho_out, float *nn_out, cudaStream_t st)
+{
+    SphArgs a;
+    a.lo = t->node_lo; a.hi = t->node_hi; a.info = t->node_info;
+    a.node_first = t->node_first; a.node_count = t->node_count; a.first_child = t->node_first_child;
+    a.nchild = t->node_nchild;
+    a.spos = t->spos; a.inv_perm = t->inv_perm; a.perm = t->perm;
+    a.active_idx = active_idx; a.h_guess = h_guess;
+    a.h_out = h_out; a.rho_out = rho_out; a.nn_out = nn_out;
+    a.n = (uint32_t)t->n; a.n_active = (uint32_t)n_active;
+    a.L = t->box; a.invL = 1.0f / t->box; a.n_des = n_des; a.tol_n = tol_n;
+    a.status = t->d_status;
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sph_density, SPH_WARPS * 32, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    const uint64_t want = (n_active + SPH_WARPS - 1) / SPH_WARPS;
+    const uint64_t cap = (uint64_t)per_sm * (uint64_t)t->sm_count;
+    const unsigned grid = (unsigned)(want < cap ? want : cap);
+    k_sph_density<<<grid, SPH_WARPS * 32, 0, st>>>(a);
+    return cudaGetLastError();
+}
