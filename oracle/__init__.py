@@ -282,6 +282,41 @@ def direct(pos, mass, eps, params: Params, target_idx=None):
     return acc, pot
 
 
+def walk_ext(tree: Tree, tpos, th, a_old=None, params: Params | None = None, want_counters: bool = False):
+    """Row f4: the walk of `tree` for targets that are not its particles (imported from another domain): tpos f32[n_t][3],
+    th f32[n_t] (= 2.8 eps of the target), a_old f32[n_t] or None.  Nothing is excluded.  -> acc, pot, counters"""
+    prm = params if params is not None else tree.params
+    tpos = _c(tpos, np.float32)
+    th = _c(th, np.float32)
+    nt = tpos.shape[0]
+    if a_old is not None:
+        a_old = _c(a_old, np.float32)
+        assert a_old.shape[0] == nt
+    acc = np.zeros((nt, 3), np.float64)
+    pot = np.zeros(nt, np.float64)
+    cnt = np.zeros((nt, NCOUNT), np.uint64) if want_counters else None
+    lib().orc_walk_ext(C.byref(prm), C.c_uint64(nt), _p(tpos), _p(th), _p(a_old), _p(tree.n_child),
+                       _p(tree.first), _p(tree.count), _p(tree.first_child), _p(tree.M), _p(tree.s),
+                       _p(tree.c), _p(tree.l), _p(tree.hmax), _p(tree.lo), _p(tree.hi),
+                       _p(tree.spos), _p(tree.smass), _p(tree.sh), _p(acc), _p(pot), _p(cnt))
+    return acc, pot, cnt
+
+
+def direct_ext(pos, mass, eps, params: Params, tpos, teps):
+    """O(N n_t) direct short-range sum on targets that are not among the sources. -> acc, pot"""
+    pos = _c(pos, np.float32)
+    mass = _c(mass, np.float32)
+    h = particle_h(_c(eps, np.float32))
+    tpos = _c(tpos, np.float32)
+    th = particle_h(_c(teps, np.float32))
+    nt = tpos.shape[0]
+    acc = np.zeros((nt, 3), np.float64)
+    pot = np.zeros(nt, np.float64)
+    lib().orc_direct_ext(C.byref(params), C.c_uint64(pos.shape[0]), _p(pos), _p(mass), _p(h), C.c_uint64(nt),
+                         _p(tpos), _p(th), _p(acc), _p(pot))
+    return acc, pot
+
+
 def algorithmic_flops(counters: np.ndarray, with_pot: bool = True) -> np.ndarray:
     """F_alg per target from the walk counters (SURVEY.md Sec. 8.4 weights).
     -> (F_alg, F_int) arrays; F_int = interaction-only part (last four terms)."""

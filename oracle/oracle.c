@@ -498,3 +498,57 @@ void orc_direct(const orc_params *p, uint64_t n, const float *pos, const float *
         if (pot) pot[t] = ph;
     }
 }
+
+/* ------------------------------------------------------------------------- */
+/* Row f4 ("secondary" phase): the same  */
+/* walk (orc_visit, unchanged) and the same direct sum for targets that are NOT */
+/* particles of the tree -- targets imported from another domain.  A target is  */
+/* (x, h, a_old); nothing is excluded (no particle of this tree is the target). */
+/* ------------------------------------------------------------------------- */
+void orc_walk_ext(const orc_params *p, uint64_t n_targets, const float *tpos, const float *th,
+                  const float *a_old, const uint8_t *n_child, const uint32_t *first,
+                  const uint32_t *count, const uint32_t *first_child, const float *M32,
+                  const float *s32, const float *c32, const float *l32, const float *hmax32,
+                  const float *lo32, const float *hi32, const float *spos, const float *smass,
+                  const float *sh, double *acc, double *pot, uint64_t *counters)
+{
+    const orc_derived D = orc_derive(p);
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t t = 0; t < (int64_t)n_targets; ++t) {
+        orc_walk_ctx W;
+        memset(&W, 0, sizeof(W));
+        W.D = &D; W.n_child = n_child; W.first = first; W.count = count;
+        W.first_child = first_child; W.M32 = M32; W.s32 = s32; W.c32 = c32; W.l32 = l32;
+        W.hmax32 = hmax32; W.lo32 = lo32; W.hi32 = hi32; W.spos = spos; W.smass = smass;
+        W.sh = sh;
+        for (int k = 0; k < 3; ++k) W.x[k] = (double)tpos[3 * t + k];
+        W.h_i = (double)th[t];
+        W.self_slot = 0xffffffffu;   /* no slot of the tree is the target */
+        W.geometric = (a_old == NULL);
+        W.A = a_old ? D.alpha * (double)a_old[t] : 0.0;
+        orc_visit(&W, 0);
+        acc[3 * t] = W.acc[0]; acc[3 * t + 1] = W.acc[1]; acc[3 * t + 2] = W.acc[2];
+        if (pot) pot[t] = W.pot;
+        if (counters)
+            for (int c = 0; c < ORC_NCOUNT; ++c) counters[ORC_NCOUNT * t + c] = W.cnt[c];
+    }
+}
+
+void orc_direct_ext(const orc_params *p, uint64_t n, const float *pos, const float *mass,
+                    const float *h, uint64_t n_targets, const float *tpos, const float *th,
+                    double *acc, double *pot)
+{
+    const orc_derived D = orc_derive(p);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t t = 0; t < (int64_t)n_targets; ++t) {
+        const double x[3] = {(double)tpos[3 * t], (double)tpos[3 * t + 1], (double)tpos[3 * t + 2]};
+        double a[3] = {0.0, 0.0, 0.0}, ph = 0.0;
+        for (uint64_t j = 0; j < n; ++j) {
+            const double xj[3] = {(double)pos[3 * j], (double)pos[3 * j + 1],
+                                  (double)pos[3 * j + 2]};
+            orc_pair(&D, x, (double)th[t], xj, (double)mass[j], (double)h[j], a, &ph);
+        }
+        acc[3 * t] = a[0]; acc[3 * t + 1] = a[1]; acc[3 * t + 2] = a[2];
+        if (pot) pot[t] = ph;
+    }
+}
