@@ -596,6 +596,89 @@ def run_sph(args):
     return 0
 
 
+def run_let(args):
+    """--scaling let (row f4, DESIGN.md Sec. 13): ONE box split over the ranks by Morton ranges of whole level-5 cells;
+    every step = domain decomposition (particles moved to their owners) + one tree per rank + primary walk + export of the
+    targets within r_cut of another domain + secondary walk there + results sent back and summed.  Under torchrun the
+    exchanges are NCCL all-to-all / all-gather (one process per GPU); with one process, --let-domains R runs the R domains
+    one after the other on this GPU (no rank waits on another) and the time is the SUM over the domains: it measures the
+    work the decomposition adds, not a speed-up."""
+    import torch
+    from paper_2606_17145_b200 import binding as B
+    from paper_2606_17145_b200 import let
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    world, rank, local = dist_setup(args.gpus, "nccl")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    w = W.make(args.workload)
+    if world > 1:
+        ex, R, mine = let.DistExchange(), world, [rank]
+    else:
+        R = max(1, args.let_domains)
+        ex, mine = let.LocalExchange(R), list(range(R))
+    prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8)
+    active = np.zeros(w.n, bool)
+    active[np.arange(w.n) if w.active_idx is None else w.active_idx] = True
+
+    def parts(a_old_pp):
+        out = {}
+        for r in mine:                                       # initial distribution: round robin over the ranks
+            sel = np.arange(r, w.n, R)
+            out[r] = let.Domain(*(torch.from_numpy(x[sel]).to(dev) for x in (w.pos, w.mass, w.eps)),
+                                torch.from_numpy(sel.astype(np.int64)).to(dev), torch.from_numpy(active[sel]).to(dev),
+                                None if a_old_pp is None else a_old_pp[torch.from_numpy(sel).to(dev)].contiguous())
+        return out
+
+    # a_old (R23 / R53): |a| of an untimed geometric pass of the same pipeline, scattered to a per-particle array
+    doms, _ = let.decompose(B, parts(None), ex, w.L)
+    res, _ = let.let_forces(B, doms, ex, w.L, prm, geometric=True, want_pot=False)
+    a_pp = torch.zeros(w.n, device=dev)
+    for r in mine:
+        a_pp[doms[r].gid[doms[r].active.long()]] = torch.linalg.vector_norm(res[r][0], dim=1)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(a_pp)
+    start = parts(a_pp)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step():
+        d, _ = let.decompose(B, start, ex, w.L)
+        out, info = let.let_forces(B, d, ex, w.L, prm)
+        return d, out, info
+
+    for _ in range(max(args.warmup, 1)):
+        step()
+    barrier(); torch.cuda.synchronize()
+    e0, e1 = ev(), ev()
+    e0.record()
+    per_step = []
+    for _ in range(args.steps):
+        es = ev(); es.record()
+        d, out, info = step()
+        per_step.append(es)
+    e1.record()
+    torch.cuda.synchronize(); barrier()
+    per_step = [a.elapsed_time(b) for a, b in zip(per_step, per_step[1:] + [e1])]
+    ms = all_max(e0.elapsed_time(e1) / args.steps, dev)
+    n_act = all_gather_int(sum(int(d[r].active.shape[0]) for r in mine), dev)
+    n_loc = all_gather_int(sum(int(d[r].pos.shape[0]) for r in mine), dev)
+    n_exp = all_gather_int(sum(v for (r, q), v in info["n_exported"].items() if r in mine), dev)
+    chk = all_gather_int(int(sum(float(out[r][0].abs().sum().item()) for r in mine) * 1e3), dev)
+    if rank == 0:
+        line = {"mode": "let", "metric": "short-range tree-gravity particles/s, one box decomposed over the ranks (decomposition + "
+                "tree per domain + primary walk + export / secondary walk + sum) on B200", "value": aggregate(n_act, ms),
+                "unit": "particles/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+                "higher_is_better": True, "scaling": "strong", "dtype": "f32", "data": "synthetic",
+                "config": {"workload": w.name, "n": w.n, "n_active": int(active.sum()), "domains": R,
+                           "exchange": "nccl all-to-all, one process per GPU" if world > 1 else
+                           f"{R} domains one after the other on one GPU (time = sum over the domains)"},
+                "particles_per_domain": n_loc if world > 1 else [int(d[r].pos.shape[0]) for r in mine],
+                "ms_each_step_rank0": per_step, "ms_median_step_rank0": sorted(per_step)[len(per_step) // 2], "exported_target_copies": int(sum(n_exp)), "checksum_sum_abs_acc_milli": int(sum(chk))}
+        print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -606,7 +689,8 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1 << 17)
     ap.add_argument("--ref-sample", type=int, default=1 << 15)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+    ap.add_argument("--let-domains", type=int, default=4, help="--scaling let with one process: number of domains emulated")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong", "let"],
                     help="weak (default): one independent box per GPU; strong: one box, every rank builds the tree and walks "
                          "a Morton range of the active targets (SURVEY.md Sec. 8.5)")
     ap.add_argument("--timesteps", type=int, default=0,
@@ -619,6 +703,8 @@ def main():
         return run_timesteps(args)
     if args.sph > 0:
         return run_sph(args)
+    if args.scaling == "let":
+        return run_let(args)
     if args.warmup < 3:
         args.warmup = 3 if args.impl == "ours" else args.warmup
     if args.impl == "reference":

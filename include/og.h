@@ -293,6 +293,42 @@ int og_ts_kick(float *vel, uint8_t *bin, float *a_old, const uint32_t *active_id
 int og_sph_density(const og_tree *tree, const uint32_t *active_idx, uint64_t n_active, float n_des, float tol_n,
                    const float *h_guess, float *h_out, float *rho_out, float *nn_out, og_stream stream);
 
+/* ---- row f4: domain-decomposed short-range force (several GPUs, one tree per domain) ---------- */
+
+/*
+ * "the tree walk is executed for particles that reside on the same MPI rank ('primary') ... particles
+ * that require tree nodes of other MPI ranks are exported ... ('secondary')", :80 (export buffers).  Readings R49..R53
+ * (DESIGN.md Sec. 13): domains are contiguous Morton ranges made of whole level-5 cells (the top 15 key bits); every
+ * domain builds the tree of its own particles in the full box (og_tree_build); the force on a target is the sum of the
+ * walks of all domains' trees with the target's own (x, h, a_old): og_shortrange_accel on its home tree (self excluded),
+ * og_shortrange_accel_ext on the others, where it is an external point.  A target is exported to a domain only if it is
+ * within r_cut of one of that domain's top-cell boxes (a domain farther away contributes exactly nothing).  The ranks
+ * exchange particles, boxes, targets and results with NCCL all-to-all / all-gather in the host layer
+ * (paper_2606_17145_b200/let.py); the calls below are its device-side steps.  All pointers DEVICE unless named HOST.
+ *
+ * og_shortrange_accel_ext  walk of `tree` for n_t targets that are NOT particles of the tree: tpos f32 [n_t][3] in
+ *     [0, box), tsoft f32 [n_t] (eps; h = 2.8 eps as in the tree), a_old f32 [n_t] or NULL (geometric criterion);
+ *     acc_out f32 [n_t][3], pot_out f32 [n_t] or NULL, overwritten, in the caller's order.  Nothing is excluded.  The
+ *     targets are walked in their own Morton order, 32 per warp.  Enqueues; stream rules as og_shortrange_accel.
+ * og_domain_cell_hist      hist u32 [32768] = particles per level-5 cell of pos f32 [n][3] (overwritten).  Enqueues.
+ * og_domain_owner          owner u32 [n] = the d with splitters[d] <= cell < splitters[d + 1]; splitters u32
+ *     [n_domains + 1], ascending, splitters[0] = 0, splitters[n_domains] = 32768.  Enqueues.
+ * og_let_export_list       list_out u32 [>= n_t] receives, ascending, the targets t with tpos[t] within r_cut (nearest
+ *     periodic image, point-to-box distance, conservative by a relative 1e-5) of one of the n_boxes <= 1024 boxes
+ *     f32 [n_boxes][6] = (lo_x, lo_y, lo_z, hi_x, hi_y, hi_z); *count_host (HOST) their number.  Synchronises `stream`.
+ * og_let_accumulate        acc[idx[k]] += part_acc[k], pot[idx[k]] += part_pot[k] for k < m (idx u32 [m], distinct,
+ *     < n; pot / part_pot may be NULL).  Enqueues.
+ */
+int og_shortrange_accel_ext(const og_tree *tree, const float *tpos, const float *tsoft, uint64_t n_t, const float *a_old,
+                            float *acc_out, float *pot_out, og_stream stream);
+int og_domain_cell_hist(const float *pos, uint64_t n, float box, uint32_t *hist, og_stream stream);
+int og_domain_owner(const float *pos, uint64_t n, float box, const uint32_t *splitters, uint32_t n_domains,
+                    uint32_t *owner, og_stream stream);
+int og_let_export_list(const float *tpos, uint64_t n_t, const float *boxes, uint32_t n_boxes, float r_cut, float box,
+                       uint32_t *list_out, uint64_t *count_host, og_stream stream);
+int og_let_accumulate(float *acc, float *pot, const uint32_t *idx, const float *part_acc, const float *part_pot,
+                      uint64_t m, uint64_t n, og_stream stream);
+
 /* Returns the device memory that freed trees / finished calls left cached in the library's
  * stream-ordered pool of the current device to the driver (the pool keeps arenas for reuse by
  * the next og_tree_build; a host code that needs the memory for something else calls this).

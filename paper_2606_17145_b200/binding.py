@@ -120,6 +120,16 @@ def _load():
     lib.og_ts_next_tick.argtypes = [vp, u64, u64, C.c_uint32, C.POINTER(u64), vp, C.c_size_t, vp]
     lib.og_ts_active_list.restype = C.c_int
     lib.og_ts_active_list.argtypes = [vp, u64, u64, C.c_uint32, vp, C.POINTER(u64), vp, C.c_size_t, vp]
+    lib.og_shortrange_accel_ext.restype = C.c_int
+    lib.og_shortrange_accel_ext.argtypes = [vp, vp, vp, u64, vp, vp, vp, vp]
+    lib.og_domain_cell_hist.restype = C.c_int
+    lib.og_domain_cell_hist.argtypes = [vp, u64, C.c_float, vp, vp]
+    lib.og_domain_owner.restype = C.c_int
+    lib.og_domain_owner.argtypes = [vp, u64, C.c_float, vp, C.c_uint32, vp, vp]
+    lib.og_let_export_list.restype = C.c_int
+    lib.og_let_export_list.argtypes = [vp, u64, vp, C.c_uint32, C.c_float, C.c_float, vp, C.POINTER(C.c_uint64), vp]
+    lib.og_let_accumulate.restype = C.c_int
+    lib.og_let_accumulate.argtypes = [vp, vp, vp, vp, vp, u64, u64, vp]
     lib.og_sph_density.restype = C.c_int
     lib.og_sph_density.argtypes = [vp, u32p, u64, C.c_float, C.c_float, vp, vp, vp, vp, vp]
     lib.og_ts_kick.restype = C.c_int
@@ -133,7 +143,8 @@ EXPORTS = ("og_tree_workspace_bytes", "og_tree_build", "og_shortrange_accel", "o
            "og_tree_stats", "og_tree_free", "og_last_error", "og_morton_keys", "og_radix_sort_scratch_bytes",
            "og_radix_sort_pairs", "og_shortrange_accel_host", "og_trim", "og_pm_create", "og_pm_longrange",
            "og_pm_free", "og_ts_scratch_bytes", "og_ts_drift", "og_ts_next_tick", "og_ts_active_list", "og_ts_kick",
-           "og_sph_density")
+           "og_sph_density", "og_shortrange_accel_ext", "og_domain_cell_hist", "og_domain_owner", "og_let_export_list",
+           "og_let_accumulate")
 
 
 def _err() -> str:
@@ -408,3 +419,50 @@ def og_sph_density(tree: Tree, n_des: float, active_idx: torch.Tensor | None = N
                                _dev(h, torch.float32, "h_out"), _dev(rho, torch.float32, "rho_out"),
                                _dev(nn, torch.float32, "nn_out"), _stream(stream)))
     return h, rho, nn
+
+
+# ---- row f4 ----------------------------------------------------------------------------------------------------------
+def og_shortrange_accel_ext(tree: Tree, tpos: torch.Tensor, tsoft: torch.Tensor, a_old: torch.Tensor | None,
+                            want_pot: bool = True, stream=None):
+    """Walk of `tree` for targets that are not its particles.  -> (acc [n_t][3], pot [n_t] | None)"""
+    nt = int(tpos.shape[0])
+    dev = tpos.device
+    acc = torch.empty((nt, 3), dtype=torch.float32, device=dev)
+    pot = torch.empty(nt, dtype=torch.float32, device=dev) if want_pot else None
+    _check(_lib.og_shortrange_accel_ext(tree.handle, _dev(tpos, torch.float32, "tpos"), _dev(tsoft, torch.float32, "tsoft"), nt,
+                                        _dev(a_old, torch.float32, "a_old"), _dev(acc, torch.float32, "acc_out"),
+                                        _dev(pot, torch.float32, "pot_out"), _stream(stream)))
+    return acc, pot
+
+
+def og_domain_cell_hist(pos: torch.Tensor, box: float, stream=None) -> torch.Tensor:
+    hist = torch.empty(1 << 15, dtype=torch.int32, device=pos.device)
+    _check(_lib.og_domain_cell_hist(_dev(pos, torch.float32, "pos"), int(pos.shape[0]), float(box),
+                                    _dev(hist, torch.int32, "hist"), _stream(stream)))
+    return hist
+
+
+def og_domain_owner(pos: torch.Tensor, box: float, splitters: torch.Tensor, stream=None) -> torch.Tensor:
+    owner = torch.empty(int(pos.shape[0]), dtype=torch.int32, device=pos.device)
+    _check(_lib.og_domain_owner(_dev(pos, torch.float32, "pos"), int(pos.shape[0]), float(box),
+                                _dev(splitters, torch.int32, "splitters"), int(splitters.shape[0]) - 1,
+                                _dev(owner, torch.int32, "owner"), _stream(stream)))
+    return owner
+
+
+def og_let_export_list(tpos: torch.Tensor, boxes: torch.Tensor, r_cut: float, box: float, stream=None) -> torch.Tensor:
+    """-> ascending int32 positions of the targets within r_cut of one of the boxes [nb][6]."""
+    nt = int(tpos.shape[0])
+    out = torch.empty(max(nt, 1), dtype=torch.int32, device=tpos.device)
+    cnt = C.c_uint64(0)
+    _check(_lib.og_let_export_list(_dev(tpos, torch.float32, "tpos"), nt, _dev(boxes, torch.float32, "boxes"),
+                                   int(boxes.shape[0]), float(r_cut), float(box), _dev(out, torch.int32, "list_out"),
+                                   C.byref(cnt), _stream(stream)))
+    return out[:int(cnt.value)]
+
+
+def og_let_accumulate(acc: torch.Tensor, pot: torch.Tensor | None, idx: torch.Tensor, part_acc: torch.Tensor,
+                      part_pot: torch.Tensor | None, stream=None):
+    _check(_lib.og_let_accumulate(_dev(acc, torch.float32, "acc"), _dev(pot, torch.float32, "pot"), _dev(idx, torch.int32, "idx"),
+                                  _dev(part_acc, torch.float32, "part_acc"), _dev(part_pot, torch.float32, "part_pot"),
+                                  int(idx.shape[0]), int(acc.shape[0]), _stream(stream)))

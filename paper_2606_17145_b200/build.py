@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libogtree.so")
 PROBE_LIB = os.path.join(HERE, "libogprobe.so")
-SOURCES = ["api.cu", "keys.cu", "radix_sort.cu", "octree.cu", "walk.cu", "pm.cu", "timestep.cu", "sph.cu"]
+SOURCES = ["api.cu", "keys.cu", "radix_sort.cu", "octree.cu", "walk.cu", "pm.cu", "timestep.cu", "sph.cu", "let.cu"]
 PROBE_SOURCES = ["probe.cu"]
 HEADERS = ["og_internal.cuh", "walk_math.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",

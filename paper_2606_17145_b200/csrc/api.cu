@@ -352,6 +352,123 @@ extern "C" int og_sph_density(const og_tree *t, const uint32_t *active_idx, uint
     return OG_OK;
 }
 
+// ---- row f4 ------------------------------------------------------------------------------------------------------
+extern "C" int og_shortrange_accel_ext(const og_tree *t, const float *tpos, const float *tsoft, uint64_t n_t,
+                                       const float *a_old, float *acc_out, float *pot_out, og_stream stream)
+{
+    g_err[0] = 0;
+    if (!t) { og_set_error("tree is NULL"); return OG_ERR_INVALID_ARG; }
+    if (n_t == 0) return OG_OK;
+    if (!tpos || !tsoft || !acc_out) { og_set_error("tpos / tsoft / acc_out must be non-NULL device pointers"); return OG_ERR_INVALID_ARG; }
+    if (n_t >= (1ull << 31)) { og_set_error("n_t out of range"); return OG_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (st != t->build_stream) OG_CUDA_TRY(cudaStreamWaitEvent(st, t->ev_built, 0), return OG_ERR_CUDA);
+    if (t->walked) OG_CUDA_TRY(cudaStreamWaitEvent(st, t->ev_walked, 0), return OG_ERR_CUDA);
+    // Morton order of the imported targets, so that a warp's 32 targets are neighbours (as for the tree's own particles)
+    const size_t nt = (size_t)n_t;
+    const size_t o_k0 = 0, o_k1 = align_up(nt * 8), o_v0 = o_k1 + align_up(nt * 8), o_v1 = o_v0 + align_up(nt * 4),
+                 o_ext = o_v1 + align_up(nt * 4), o_sc = o_ext + align_up(nt * 16),
+                 total = o_sc + align_up(ogk_sort_scratch_bytes(n_t));
+    char *tmp = nullptr;
+    cudaError_t e = og_malloc_async((void **)&tmp, total, st);
+    if (e != cudaSuccess) {
+        og_set_error("cudaMallocAsync(%zu bytes) failed: %s", total, cudaGetErrorString(e));
+        (void)cudaGetLastError();
+        return OG_ERR_OUT_OF_MEMORY;
+    }
+    uint64_t *k0 = (uint64_t *)(tmp + o_k0), *k1 = (uint64_t *)(tmp + o_k1);
+    uint32_t *v0 = (uint32_t *)(tmp + o_v0), *v1 = (uint32_t *)(tmp + o_v1);
+    float4 *ext = (float4 *)(tmp + o_ext);
+    int in_alt = 0;
+#define OG_EXT_TRY(expr) OG_CUDA_TRY(expr, { cudaFreeAsync(tmp, st); return OG_ERR_CUDA; })
+    OG_EXT_TRY(ogk_keys(tpos, n_t, t->box, k0, v0, t->d_status, (t->prm.flags & OG_VALIDATE_POS) != 0, st));
+    OG_EXT_TRY(ogk_radix_sort(k0, v0, k1, v1, n_t, 0, 64, tmp + o_sc, &in_alt, st));
+    const uint32_t *order = in_alt ? v1 : v0;
+    OG_EXT_TRY(ogk_ext_gather(tpos, tsoft, order, n_t, ext, st));
+    OG_EXT_TRY(ogk_walk(t, nullptr, order, n_t, a_old, acc_out, pot_out, st, ext));
+    OG_EXT_TRY(cudaEventRecord(t->ev_walked, st));
+    t->walked = true;
+    OG_EXT_TRY(cudaFreeAsync(tmp, st));
+#undef OG_EXT_TRY
+    return OG_OK;
+}
+
+static int domain_keys(const float *pos, uint64_t n, float box, uint64_t **keys, cudaStream_t st)
+{
+    *keys = nullptr;
+    if (n == 0) return OG_OK;
+    if (!pos || !(box > 0.0f) || n >= (1ull << 31)) { og_set_error("bad pos / box / n"); return OG_ERR_INVALID_ARG; }
+    cudaError_t e = og_malloc_async((void **)keys, n * sizeof(uint64_t), st);
+    if (e != cudaSuccess) { og_set_error("cudaMallocAsync failed: %s", cudaGetErrorString(e)); (void)cudaGetLastError(); return OG_ERR_OUT_OF_MEMORY; }
+    OG_CUDA_TRY(ogk_keys(pos, n, box, *keys, nullptr, nullptr, false, st), { cudaFreeAsync(*keys, st); return OG_ERR_CUDA; });
+    return OG_OK;
+}
+
+extern "C" int og_domain_cell_hist(const float *pos, uint64_t n, float box, uint32_t *hist, og_stream stream)
+{
+    g_err[0] = 0;
+    if (!hist) { og_set_error("hist is NULL"); return OG_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    uint64_t *keys = nullptr;
+    const int rc = domain_keys(pos, n, box, &keys, st);
+    if (rc != OG_OK) return rc;
+    OG_CUDA_TRY(ogk_cell_hist(keys, n, hist, st), { if (keys) cudaFreeAsync(keys, st); return OG_ERR_CUDA; });
+    if (keys) OG_CUDA_TRY(cudaFreeAsync(keys, st), return OG_ERR_CUDA);
+    return OG_OK;
+}
+
+extern "C" int og_domain_owner(const float *pos, uint64_t n, float box, const uint32_t *splitters, uint32_t n_domains,
+                               uint32_t *owner, og_stream stream)
+{
+    g_err[0] = 0;
+    if (n == 0) return OG_OK;
+    if (!splitters || !owner || n_domains == 0) { og_set_error("splitters / owner NULL or n_domains == 0"); return OG_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    uint64_t *keys = nullptr;
+    const int rc = domain_keys(pos, n, box, &keys, st);
+    if (rc != OG_OK) return rc;
+    OG_CUDA_TRY(ogk_owner(keys, n, splitters, n_domains, owner, st), { cudaFreeAsync(keys, st); return OG_ERR_CUDA; });
+    OG_CUDA_TRY(cudaFreeAsync(keys, st), return OG_ERR_CUDA);
+    return OG_OK;
+}
+
+extern "C" int og_let_export_list(const float *tpos, uint64_t n_t, const float *boxes, uint32_t n_boxes, float r_cut,
+                                  float box, uint32_t *list_out, uint64_t *count_host, og_stream stream)
+{
+    g_err[0] = 0;
+    if (!count_host) { og_set_error("count_host is NULL"); return OG_ERR_INVALID_ARG; }
+    *count_host = 0;
+    if (n_t == 0 || n_boxes == 0) return OG_OK;
+    if (!tpos || !boxes || !list_out || n_boxes > 1024 || !(box > 0.0f) || n_t >= (1ull << 31)) {
+        og_set_error("bad tpos / boxes / list_out, or n_boxes > 1024"); return OG_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t o_sc = align_up((size_t)n_t), total = o_sc + align_up(ogk_flag_scratch_bytes(n_t));
+    char *tmp = nullptr;
+    cudaError_t e = og_malloc_async((void **)&tmp, total, st);
+    if (e != cudaSuccess) { og_set_error("cudaMallocAsync failed: %s", cudaGetErrorString(e)); (void)cudaGetLastError(); return OG_ERR_OUT_OF_MEMORY; }
+    uint32_t *total_dev = nullptr, cnt = 0;
+#define OG_LET_TRY(expr) OG_CUDA_TRY(expr, { cudaFreeAsync(tmp, st); return OG_ERR_CUDA; })
+    OG_LET_TRY(ogk_let_mark(tpos, n_t, boxes, n_boxes, r_cut, box, (uint8_t *)tmp, st));
+    OG_LET_TRY(ogk_flag_compact((const uint8_t *)tmp, n_t, list_out, (uint32_t *)(tmp + o_sc), &total_dev, st));
+    OG_LET_TRY(cudaMemcpyAsync(&cnt, total_dev, sizeof(cnt), cudaMemcpyDeviceToHost, st));
+    OG_LET_TRY(cudaStreamSynchronize(st));
+    OG_LET_TRY(cudaFreeAsync(tmp, st));
+#undef OG_LET_TRY
+    *count_host = cnt;
+    return OG_OK;
+}
+
+extern "C" int og_let_accumulate(float *acc, float *pot, const uint32_t *idx, const float *part_acc, const float *part_pot,
+                                 uint64_t m, uint64_t n, og_stream stream)
+{
+    g_err[0] = 0;
+    if (m == 0) return OG_OK;
+    if (!acc || !idx || !part_acc) { og_set_error("acc / idx / part_acc NULL"); return OG_ERR_INVALID_ARG; }
+    OG_CUDA_TRY(ogk_let_accumulate(acc, pot, idx, part_acc, part_pot, m, n, (cudaStream_t)stream), return OG_ERR_CUDA);
+    return OG_OK;
+}
+
 extern "C" int og_tree_get(const og_tree *t, int field, const void **dev_ptr, uint64_t *count)
 {
     g_err[0] = 0;

@@ -117,12 +117,24 @@ cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st);
 // a6 + a7
 cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out,
                      uint64_t n_active, const float *a_old, float *acc_out, float *pot_out,
-                     cudaStream_t st);
+                     cudaStream_t st, const float4 *ext = nullptr);
 size_t ogk_walk_spill_bytes(int sm_count, uint32_t spill_entries);
 uint32_t ogk_walk_spill_entries(const og_params *p);
 // f3
 cudaError_t ogk_sph_density(const og_tree *t, const uint32_t *active_idx, uint64_t n_active, float n_des, float tol_n,
                             const float *h_guess, float *h_out, float *rho_out, float *nn_out, cudaStream_t st);
+// f4 (let.cu)
+cudaError_t ogk_ext_gather(const float *tpos, const float *tsoft, const uint32_t *order, uint64_t n_t, float4 *ext,
+                           cudaStream_t st);
+cudaError_t ogk_cell_hist(const uint64_t *keys, uint64_t n, uint32_t *hist, cudaStream_t st);
+cudaError_t ogk_owner(const uint64_t *keys, uint64_t n, const uint32_t *S, uint32_t R, uint32_t *owner, cudaStream_t st);
+cudaError_t ogk_let_mark(const float *tpos, uint64_t n_t, const float *boxes, uint32_t nb, float r_cut, float L,
+                         uint8_t *flag, cudaStream_t st);
+size_t ogk_flag_scratch_bytes(uint64_t n);
+cudaError_t ogk_flag_compact(const uint8_t *flag, uint64_t n, uint32_t *out, uint32_t *scratch, uint32_t **total_dev,
+                             cudaStream_t st);
+cudaError_t ogk_let_accumulate(float *acc, float *pot, const uint32_t *idx, const float *pacc, const float *ppot, uint64_t m,
+                               uint64_t n, cudaStream_t st);
 // helpers for the active subset
 cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_perm, uint64_t n,
                              uint64_t n_active, uint64_t *keys, uint32_t *vals, uint32_t *d_status,

@@ -31,6 +31,8 @@ struct WalkArgs {
     const float4 *spos;
     const float *sh;
     const uint32_t *tgt_slot;  // NULL -> identity
+    const float4 *ext;         // row f4: NULL, or EXTERNAL targets (x, y, z, h) in walk order (not particles of the tree:
+                               // no slot, nothing excluded); tgt_slot is NULL then
     const uint32_t *tgt_out;   // position in the caller's order
     const float *a_old;
     float *acc_out;
@@ -62,12 +64,18 @@ __device__ __forceinline__ NodeRec load_node(const WalkArgs &a, uint32_t j)
 __device__ __forceinline__ Target load_target(const WalkArgs &a, uint32_t k, uint32_t &out, bool geom)
 {
     Target t;
-    const uint32_t slot = a.tgt_slot ? __ldg(a.tgt_slot + k) : k;
     out = __ldg(a.tgt_out + k);
-    const float4 p = __ldg(a.spos + slot);
-    t.x = p.x; t.y = p.y; t.z = p.z;
-    t.h = __ldg(a.sh + slot);
-    t.slot = slot;
+    if (a.ext != nullptr) {
+        const float4 p = __ldg(a.ext + k);
+        t.x = p.x; t.y = p.y; t.z = p.z; t.h = p.w;
+        t.slot = 0xffffffffu;      // equals no particle's slot: the self exclusion never fires
+    } else {
+        const uint32_t slot = a.tgt_slot ? __ldg(a.tgt_slot + k) : k;
+        const float4 p = __ldg(a.spos + slot);
+        t.x = p.x; t.y = p.y; t.z = p.z;
+        t.h = __ldg(a.sh + slot);
+        t.slot = slot;
+    }
     t.aold = geom ? 0.0f : __ldg(a.a_old + out);
     t.A = a.c.alpha * t.aold;
     return t;
@@ -1010,9 +1018,10 @@ size_t ogk_walk_spill_bytes(int sm_count, uint32_t spill_entries)
 }
 
 cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out, uint64_t n_active,
-                     const float *a_old, float *acc_out, float *pot_out, cudaStream_t st)
+                     const float *a_old, float *acc_out, float *pot_out, cudaStream_t st, const float4 *ext)
 {
     WalkArgs a;
+    a.ext = ext;
     a.com = t->node_com; a.cell = t->node_cell; a.lo = t->node_lo; a.hi = t->node_hi;
     a.info = t->node_info; a.rec = t->node_rec; a.spos = t->spos; a.sh = t->sh;
     a.tgt_slot = tgt_slot; a.tgt_out = tgt_out; a.a_old = a_old; a.acc_out = acc_out; a.pot_out = pot_out;
