@@ -4,10 +4,10 @@
 // a4 (C3, R5..R7): cell (l, p) = sorted slots whose key >> (63 - 3l) == p.  Root = node 0;
 // a node is a leaf iff count <= leaf_max or l == 21; otherwise it gets one child per
 // non-empty octant, ascending octant; numbering is breadth-first, so children are contiguous.
-// Built level by level in ONE persistent cooperative kernel (no host round trip): per level
-// (1) every node counts its non-empty octants by a 7-way lock-step binary search on the
-// octant digit, (2) an exclusive scan over the level gives the children's BFS indices,
-// (3) the children records are written.  Integer work only; the result is unique.
+// Built level by level in ONE persistent cooperative kernel (no host round trip), one pass and one grid
+// synchronisation per level: every node finds its non-empty octants by a 7-way lock-step binary search on
+// the octant digit, a single-pass scan (decoupled look-back over chunk totals) gives the children's BFS
+// indices, and the children records are written in the same pass.  Integer work only; the result is unique.
 //
 // a5 (C4, R8..R11): leaves sum over their slots in slot order, internal nodes over their
 // children in order, all in fp64 with separately rounded products and sums (__dmul_rn /
@@ -34,7 +34,7 @@ struct OctArgs {
     uint8_t *nchild;
     uint32_t *level_start;  // [24]
     uint32_t *status;
-    uint32_t *chunk_sums;   // [ceil(max_nodes / OCT_THREADS) + 1]
+    unsigned long long *chunk_status;   // [ceil(max_nodes / OCT_THREADS) + 1], zeroed before the launch
 };
 
 // lb[o] (o = 1..7) = number of slots of [f, f + c) whose octant digit is < o.
@@ -86,13 +86,28 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t x, uint32_t *warp_b
     return woff + incl - x;
 }
 
+// Chunk status word of the decoupled look-back scan over the children counts of a level: bits 0..31 the value,
+// bits 32..33 the flag (1 = the chunk's own total, 2 = inclusive prefix up to and including the chunk), bits 34.. a
+// tag = level + 1, so that the words left by earlier levels (and the zeroed initial state) read as "not published".
+#define OCT_FLAG_AGG 1ull
+#define OCT_FLAG_INCL 2ull
+
+__device__ __forceinline__ unsigned long long oct_ld(const unsigned long long *p)
+{
+    return *reinterpret_cast<const volatile unsigned long long *>(p);
+}
+__device__ __forceinline__ void oct_st(unsigned long long *p, unsigned long long v)
+{
+    *reinterpret_cast<volatile unsigned long long *>(p) = v;
+}
+
 __global__ void __launch_bounds__(OCT_THREADS)
 k_octree(OctArgs a)
 {
     cg::grid_group grid = cg::this_grid();
     __shared__ uint32_t warp_buf[OCT_THREADS / 32];
     __shared__ uint32_t carry_s;
-    const uint32_t tid = threadIdx.x;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, wid = tid >> 5;
     if (blockIdx.x == 0 && tid == 0) {
         a.level[0] = 0; a.first[0] = 0; a.count[0] = a.n;
         a.level_start[0] = 0;
@@ -111,70 +126,66 @@ k_octree(OctArgs a)
         }
         const int shift = 60 - 3 * lv;
         const uint32_t nchunks = (nl + OCT_THREADS - 1) / OCT_THREADS;
-        // (1) children per node, chunk sums
+        const unsigned long long tag = (unsigned long long)(lv + 1) << 34;
+        // One pass per level: every chunk of 256 nodes finds its nodes' octant boundaries (kept in registers),
+        // scans the children counts inside the chunk, obtains the number of children of all earlier chunks by a
+        // decoupled look-back over the published chunk totals, and writes its children at once.  A block takes its
+        // chunks in ascending order and all blocks are resident (cooperative launch), so the look-back always
+        // finds its predecessors in progress or done.
         for (uint32_t ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
             const uint32_t node = beg + ch * OCT_THREADS + tid;
-            uint32_t nc = 0;
+            uint32_t nc = 0, f = 0, c = 0;
+            uint32_t lb[9];
             if (node < end) {
-                const uint32_t c = a.count[node];
+                c = a.count[node];
+                f = a.first[node];
                 if (c > a.leaf_max) {
-                    uint32_t lb[9];
-                    octant_bounds(a.keys, a.first[node], c, shift, lb);
+                    octant_bounds(a.keys, f, c, shift, lb);
 #pragma unroll
                     for (int o = 0; o < 8; ++o) nc += (lb[o + 1] > lb[o]) ? 1u : 0u;
                 }
-                a.nchild[node] = (uint8_t)nc;
             }
-            uint32_t tot;
-            block_excl_scan(nc, warp_buf, &tot);
-            if (tid == 0) a.chunk_sums[ch] = tot;
-            __syncthreads();
-        }
-        grid.sync();
-        // (2) exclusive scan of the chunk sums by block 0
-        if (blockIdx.x == 0) {
-            if (tid == 0) carry_s = 0;
-            __syncthreads();
-            for (uint32_t b0 = 0; b0 < nchunks; b0 += OCT_THREADS) {
-                const uint32_t b = b0 + tid;
-                const uint32_t x = (b < nchunks) ? a.chunk_sums[b] : 0;
-                uint32_t tot;
-                const uint32_t ex = block_excl_scan(x, warp_buf, &tot);
-                const uint32_t carry = carry_s;
-                if (b < nchunks) a.chunk_sums[b] = carry + ex;
-                __syncthreads();
-                if (tid == 0) carry_s = carry + tot;
-                __syncthreads();
-            }
-            if (tid == 0) {
-                uint64_t new_end = (uint64_t)end + carry_s;
-                if (new_end > a.max_nodes) {  // R6: latch the overflow, stop splitting
-                    atomicOr(a.status, OG_DEV_NODE_OVERFLOW);
-                    new_end = end;
-                }
-                for (int k = lv + 2; k < 24; ++k) a.level_start[k] = (uint32_t)new_end;
-            }
-        }
-        grid.sync();
-        const uint32_t new_end = *((volatile uint32_t *)&a.level_start[lv + 2]);
-        const bool overflow = (*((volatile uint32_t *)a.status) & OG_DEV_NODE_OVERFLOW) != 0;
-        // (3) write the children
-        for (uint32_t ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
-            const uint32_t node = beg + ch * OCT_THREADS + tid;
-            uint32_t nc = 0;
-            if (node < end && !overflow) nc = a.nchild[node];
             uint32_t tot;
             const uint32_t off = block_excl_scan(nc, warp_buf, &tot);
+            if (wid == 0) {
+                if (lane == 0) oct_st(a.chunk_status + ch, tag | ((ch == 0 ? OCT_FLAG_INCL : OCT_FLAG_AGG) << 32) | tot);
+                uint32_t excl = 0;
+                if (ch > 0) {
+                    for (int64_t base = (int64_t)ch - 1;; base -= 32) {
+                        const int64_t idx = base - (int64_t)lane;
+                        unsigned long long sw;
+                        do {
+                            sw = (idx >= 0) ? oct_ld(a.chunk_status + idx) : (tag | (OCT_FLAG_INCL << 32));
+                        } while (!__all_sync(0xffffffffu, (sw >> 34) == (tag >> 34)));
+                        const uint32_t incl_lanes = __ballot_sync(0xffffffffu, ((sw >> 32) & 3ull) == OCT_FLAG_INCL);
+                        const uint32_t upto = incl_lanes ? (uint32_t)(__ffs(incl_lanes) - 1) : 31u;   // nearest inclusive prefix
+                        uint32_t v = (lane <= upto) ? (uint32_t)sw : 0u;
+#pragma unroll
+                        for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                        excl += v;
+                        if (incl_lanes) break;
+                    }
+                    if (lane == 0) oct_st(a.chunk_status + ch, tag | (OCT_FLAG_INCL << 32) | (excl + tot));
+                }
+                if (lane == 0) {
+                    carry_s = excl;
+                    if (ch == nchunks - 1) {   // the level's total: where the next level ends
+                        uint64_t new_end = (uint64_t)end + excl + tot;
+                        if (new_end > a.max_nodes) {  // R6: latch the overflow, stop splitting
+                            atomicOr(a.status, OG_DEV_NODE_OVERFLOW);
+                            new_end = end;
+                        }
+                        for (int k = lv + 2; k < 24; ++k) a.level_start[k] = (uint32_t)new_end;
+                    }
+                }
+            }
+            __syncthreads();
             if (node < end) {
-                if (overflow) a.nchild[node] = 0;
-                if (nc == 0) {
-                    a.first_child[node] = 0;
-                } else {
-                    uint32_t child = end + a.chunk_sums[ch] + off;
-                    a.first_child[node] = child;
-                    const uint32_t f = a.first[node], c = a.count[node];
-                    uint32_t lb[9];
-                    octant_bounds(a.keys, f, c, shift, lb);
+                uint32_t child = end + carry_s + off;
+                const bool fits = (uint64_t)child + nc <= (uint64_t)a.max_nodes;   // (else the level is undone below)
+                a.nchild[node] = (uint8_t)(fits ? nc : 0u);
+                a.first_child[node] = (nc && fits) ? child : 0u;
+                if (nc && fits) {
 #pragma unroll
                     for (int o = 0; o < 8; ++o) {
                         const uint32_t cc = lb[o + 1] - lb[o];
@@ -187,12 +198,19 @@ k_octree(OctArgs a)
                     }
                 }
             }
-            __syncthreads();
+            __syncthreads();   // carry_s, warp_buf are reused by the block's next chunk
         }
-        if (overflow) break;
+        grid.sync();
+        const uint32_t new_end = *((volatile uint32_t *)&a.level_start[lv + 2]);
+        if ((*((volatile uint32_t *)a.status) & OG_DEV_NODE_OVERFLOW) != 0) {
+            // the node capacity is exceeded at this level: its nodes stay leaves (the status is latched)
+            for (uint32_t j = beg + blockIdx.x * OCT_THREADS + tid; j < end; j += gridDim.x * OCT_THREADS) {
+                a.nchild[j] = 0; a.first_child[j] = 0;
+            }
+            break;
+        }
         beg = end;
         end = new_end;
-        grid.sync();
     }
 }
 
@@ -346,20 +364,22 @@ int coop_grid(const void *kernel, int threads, int sm_count)
 size_t ogk_octree_scratch_bytes(uint32_t max_nodes)
 {
     const size_t chunks = ((size_t)max_nodes + OCT_THREADS - 1) / OCT_THREADS + 1;
-    return ((chunks * sizeof(uint32_t) + 255) & ~(size_t)255) + (size_t)max_nodes * sizeof(double4);
+    return ((chunks * sizeof(unsigned long long) + 255) & ~(size_t)255) + (size_t)max_nodes * sizeof(double4);
 }
 
 cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st)
 {
     const size_t chunks = ((size_t)t->max_nodes + OCT_THREADS - 1) / OCT_THREADS + 1;
-    uint32_t *chunk_sums = reinterpret_cast<uint32_t *>(scratch);
+    unsigned long long *chunk_status = reinterpret_cast<unsigned long long *>(scratch);
     double4 *sums = reinterpret_cast<double4 *>(reinterpret_cast<char *>(scratch) +
-                                                ((chunks * sizeof(uint32_t) + 255) & ~(size_t)255));
+                                                ((chunks * sizeof(unsigned long long) + 255) & ~(size_t)255));
+    cudaError_t e = cudaMemsetAsync(chunk_status, 0, chunks * sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
     OctArgs oa{t->keys, (uint32_t)t->n, t->prm.leaf_max, t->max_nodes, t->node_level, t->node_first,
                t->node_count, t->node_first_child, t->node_nchild, t->d_level_start, t->d_status,
-               chunk_sums};
+               chunk_status};
     void *args1[] = {&oa};
-    cudaError_t e = cudaLaunchCooperativeKernel((const void *)k_octree,
+    e = cudaLaunchCooperativeKernel((const void *)k_octree,
                                                 dim3(coop_grid((const void *)k_octree, OCT_THREADS, t->sm_count)),
                                                 dim3(OCT_THREADS), args1, 0, st);
     if (e != cudaSuccess) return e;
