@@ -679,6 +679,50 @@ def run_let(args):
     return 0
 
 
+def run_pm(args):
+    """--pm NG (row f1): og_pm_longrange on the workload (all particles sources and targets) with an
+    NG^3 mesh and the workload's r_s.  HBM-bound: the line carries the achieved fraction of the measured copy bandwidth for
+    the compulsory traffic (particles in, results out, every grid once per pass over it)."""
+    import torch
+    from paper_2606_17145_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    w = W.make(args.workload)
+    ng = int(args.pm)
+    pos, mass = torch.from_numpy(w.pos).to(dev), torch.from_numpy(w.mass).to(dev)
+    pm = B.og_pm_create(ng, w.L, w.r_s, w.G)
+    for _ in range(max(args.warmup, 1)):
+        acc, pot = B.og_pm_longrange(pm, pos, mass)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        acc, pot = B.og_pm_longrange(pm, pos, mass)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    peaks, src = measured_peaks()
+    g = float(ng) ** 3
+    # deposit: 16 B in per particle + the mass grid written once; R2C + C2R: each grid read and written once per FFT
+    # (two real grids of 4 B, one complex of ~4 B per point); Green: complex grid read + written; gradient: potential
+    # read, float4 written; interpolation: 12 B position + 16 B out per target (the 8 x 16 B gathers hit L2)
+    bytes_alg = w.n * 16.0 + g * 4.0 + 2.0 * (g * 4.0 + g * 4.0) + 2.0 * g * 4.0 + (g * 4.0 + g * 16.0) + w.n * 28.0
+    hbm = peaks.get("hbm_gbs", 0.0)
+    line = {"mode": "pm_longrange", "metric": "PM long-range force particles/s (CIC deposit + cuFFT + Green + gradient + CIC "
+            "interpolation) on B200", "value": w.n / (ms * 1e-3), "unit": "particles/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "n": w.n, "ng": ng, "r_s": w.r_s, "box": w.L},
+            "roofline": {"bound": "hbm", "achieved": bytes_alg / (ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                         "frac": (bytes_alg / (ms * 1e-3) / 1e9 / hbm) if hbm else None, "traffic": None,
+                         "algorithmic_bytes": bytes_alg, "peak_source": src},
+            "checksum_mean_abs_acc": float(acc.abs().mean().item())}
+    B.og_pm_free(pm)
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -695,12 +739,15 @@ def main():
                          "a Morton range of the active targets (SURVEY.md Sec. 8.5)")
     ap.add_argument("--timesteps", type=int, default=0,
                     help="row f2: run this many synchronisation steps of the time-step shell instead of the standard step")
+    ap.add_argument("--pm", type=int, default=0, help="row f1: time og_pm_longrange with an NG^3 mesh instead of the standard step")
     ap.add_argument("--sph", type=float, default=0.0,
                     help="row f3: time og_sph_density with this desired neighbour number instead of the standard step")
     ap.add_argument("--sph-cpu-sample", type=int, default=300)
     args = ap.parse_args()
     if args.timesteps > 0:
         return run_timesteps(args)
+    if args.pm > 0:
+        return run_pm(args)
     if args.sph > 0:
         return run_sph(args)
     if args.scaling == "let":
