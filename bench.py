@@ -569,11 +569,18 @@ def run_sph(args):
     ms_cold, h, rho, nn = timed(None)
     ms_warm, h2, _, _ = timed(h.clone())
     status = B.og_tree_status(tree)
+    n_nodes = float(B.og_tree_stats(tree)["n_nodes"])
     line = {"mode": "sph_density", "metric": "SPH density + smoothing-length targets/s (neighbour walk + root of N(h) = n_des) on B200",
             "value": w.n / (ms_cold * 1e-3), "unit": "particles/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_cold, "ms_per_step_with_h_guess": ms_warm, "value_with_h_guess": w.n / (ms_warm * 1e-3),
             "higher_is_better": True, "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "n": w.n, "n_des": n_des, "tol_n": 0.0, "box": w.L},
+            "roofline": {"bound": "hbm", "achieved": (w.n * 28.0 + n_nodes * 40.0) / (ms_cold * 1e-3) / 1e9,
+                         "peak": measured_peaks()[0].get("hbm_gbs", 0.0), "unit": "GB/s",
+                         "frac": (w.n * 28.0 + n_nodes * 40.0) / (ms_cold * 1e-3) / 1e9 / max(measured_peaks()[0].get("hbm_gbs", 1.0), 1.0),
+                         "traffic": None, "note": "compulsory bytes only (every particle 16 B and every node's AABB + info 40 B "
+                         "once, 12 B out per target; leaf_max 8): the kernel is a latency-bound walk, "
+                         "one target per warp, far from either roofline (DESIGN.md Sec. 12)"},
             "checks": {"mean_N": float(nn.mean().item()), "max_abs_N_minus_n_des": float((nn - n_des).abs().max().item()),
                        "max_rel_h_warm_vs_cold": float(((h2 - h).abs() / h).max().item()), "mean_h": float(h.mean().item())},
             "status": status}

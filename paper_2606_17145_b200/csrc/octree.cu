@@ -244,14 +244,49 @@ __device__ __forceinline__ uint32_t og_compact3(uint64_t x)
     return (uint32_t)x;
 }
 
-__device__ __forceinline__ void up_store(const UpArgs &a, uint32_t j, double M, double ax, double ay,
-                                         double az, float3 lo, float3 hi, float hm)
+// Writes every record of a finished node: the fp64 sums (read by the parent), the fp32 records (R9) and the packed
+// walk record n0, n1, n2 (og_internal.cuh).  R and ng are bounds used only by conservative tests of the walk, so they
+// are rounded up.
+__device__ __forceinline__ void up_store(const UpArgs &a, uint32_t j, int lv, float4 cc, uint2 info, double M, double ax,
+                                         double ay, double az, float3 lo, float3 hi, float hm)
 {
     a.sums[j] = make_double4(M, ax, ay, az);
-    a.com[j] = make_float4(__double2float_rn(__ddiv_rn(ax, M)), __double2float_rn(__ddiv_rn(ay, M)),
-                           __double2float_rn(__ddiv_rn(az, M)), __double2float_rn(M));
+    const float4 s = make_float4(__double2float_rn(__ddiv_rn(ax, M)), __double2float_rn(__ddiv_rn(ay, M)),
+                                 __double2float_rn(__ddiv_rn(az, M)), __double2float_rn(M));
+    a.com[j] = s;
+    a.cell[j] = cc;
+    a.info[j] = info;
     a.lo[j] = make_float4(lo.x, lo.y, lo.z, hm);
     a.hi[j] = make_float4(hi.x, hi.y, hi.z, 0.0f);
+    const double ex = fmax((double)s.x - (double)lo.x, (double)hi.x - (double)s.x),
+                 ey = fmax((double)s.y - (double)lo.y, (double)hi.y - (double)s.y),
+                 ez = fmax((double)s.z - (double)lo.z, (double)hi.z - (double)s.z);
+    const float R = __double2float_ru(sqrt(ex * ex + ey * ey + ez * ez) * (1.0 + 1e-6));
+    const double lim = 0.6 * (double)cc.w;
+    const double gx = lim + fabs((double)s.x - (double)cc.x), gy = lim + fabs((double)s.y - (double)cc.y),
+                 gz = lim + fabs((double)s.z - (double)cc.z);
+    const float rg = __double2float_ru(sqrt(gx * gx + gy * gy + gz * gz) * (1.0 + 1e-6));
+    const uint32_t leaf = (info.y & OG_LEAF_BIT) ? 1u : 0u;
+    const uint32_t cnt = info.y & ~OG_LEAF_BIT;
+    if (cnt >= (1u << 26)) atomicOr(a.status, OG_DEV_NODE_OVERFLOW);   // does not fit the packed record
+    const uint32_t meta = ((uint32_t)lv << 27) | (leaf << 26) | (cnt & 0x03ffffffu);
+    uint4 *r = a.rec + 3 * (size_t)j;
+    r[0] = make_uint4(__float_as_uint(s.x), __float_as_uint(s.y), __float_as_uint(s.z), __float_as_uint(s.w));
+    r[1] = make_uint4(__float_as_uint(R), __float_as_uint(fmaxf(rg, hm)), info.x, meta);
+    r[2] = make_uint4(__float_as_uint(cc.x), __float_as_uint(cc.y), __float_as_uint(cc.z), __float_as_uint(hm));
+}
+
+// geometric centre and side of the cell of node (level lv, first slot f): (c_x, c_y, c_z, l)
+__device__ __forceinline__ float4 up_cell(const UpArgs &a, int lv, uint32_t f)
+{
+    const uint64_t key = __ldg(a.keys + f);
+    const double l = ldexp((double)a.box, -lv);
+    const int sh = OG_MAX_LEVEL - lv;
+    const uint32_t px = lv ? (og_compact3(key >> 2) >> sh) : 0u;
+    const uint32_t py = lv ? (og_compact3(key >> 1) >> sh) : 0u;
+    const uint32_t pz = lv ? (og_compact3(key) >> sh) : 0u;
+    return make_float4(__double2float_rn(__dmul_rn((double)px + 0.5, l)), __double2float_rn(__dmul_rn((double)py + 0.5, l)),
+                       __double2float_rn(__dmul_rn((double)pz + 0.5, l)), __double2float_rn(l));
 }
 
 __global__ void __launch_bounds__(OCT_THREADS)
@@ -261,42 +296,29 @@ k_upward(UpArgs a)
     const uint32_t n_nodes = a.level_start[22];
     const uint32_t stride = gridDim.x * OCT_THREADS;
     const uint32_t t0 = blockIdx.x * OCT_THREADS + threadIdx.x;
-    // (A) every node: geometry + info; leaves: sums over their slots in slot order
+    // (A) leaves (every level at once): sums over their slots in slot order, all records
     for (uint32_t j = t0; j < n_nodes; j += stride) {
+        if (a.nchild[j] != 0) continue;
         const int lv = a.level[j];
-        const uint32_t f = a.first[j], c = a.count[j], nc = a.nchild[j];
-        const uint64_t key = __ldg(a.keys + f);
-        const double l = ldexp((double)a.box, -lv);
-        const int sh = OG_MAX_LEVEL - lv;
-        const uint32_t px = lv ? (og_compact3(key >> 2) >> sh) : 0u;
-        const uint32_t py = lv ? (og_compact3(key >> 1) >> sh) : 0u;
-        const uint32_t pz = lv ? (og_compact3(key) >> sh) : 0u;
-        a.cell[j] = make_float4(__double2float_rn(__dmul_rn((double)px + 0.5, l)),
-                                __double2float_rn(__dmul_rn((double)py + 0.5, l)),
-                                __double2float_rn(__dmul_rn((double)pz + 0.5, l)), __double2float_rn(l));
-        if (nc == 0) {
-            a.info[j] = make_uint2(f, c | OG_LEAF_BIT);
-            double M = 0.0, ax = 0.0, ay = 0.0, az = 0.0;
-            float4 p = __ldg(a.spos + f);
-            float3 lo = make_float3(p.x, p.y, p.z), hi = lo;
-            float hm = __ldg(a.sh + f);
-            for (uint32_t s = f; s < f + c; ++s) {
-                p = __ldg(a.spos + s);
-                const double m = (double)p.w;
-                M = __dadd_rn(M, m);
-                ax = __dadd_rn(ax, __dmul_rn(m, (double)p.x));
-                ay = __dadd_rn(ay, __dmul_rn(m, (double)p.y));
-                az = __dadd_rn(az, __dmul_rn(m, (double)p.z));
-                lo.x = fminf(lo.x, p.x); lo.y = fminf(lo.y, p.y); lo.z = fminf(lo.z, p.z);
-                hi.x = fmaxf(hi.x, p.x); hi.y = fmaxf(hi.y, p.y); hi.z = fmaxf(hi.z, p.z);
-                hm = fmaxf(hm, __ldg(a.sh + s));
-            }
-            up_store(a, j, M, ax, ay, az, lo, hi, hm);
-        } else {
-            a.info[j] = make_uint2(a.first_child[j], nc);
+        const uint32_t f = a.first[j], c = a.count[j];
+        double M = 0.0, ax = 0.0, ay = 0.0, az = 0.0;
+        float4 p = __ldg(a.spos + f);
+        float3 lo = make_float3(p.x, p.y, p.z), hi = lo;
+        float hm = __ldg(a.sh + f);
+        for (uint32_t s = f; s < f + c; ++s) {
+            p = __ldg(a.spos + s);
+            const double m = (double)p.w;
+            M = __dadd_rn(M, m);
+            ax = __dadd_rn(ax, __dmul_rn(m, (double)p.x));
+            ay = __dadd_rn(ay, __dmul_rn(m, (double)p.y));
+            az = __dadd_rn(az, __dmul_rn(m, (double)p.z));
+            lo.x = fminf(lo.x, p.x); lo.y = fminf(lo.y, p.y); lo.z = fminf(lo.z, p.z);
+            hi.x = fmaxf(hi.x, p.x); hi.y = fmaxf(hi.y, p.y); hi.z = fmaxf(hi.z, p.z);
+            hm = fmaxf(hm, __ldg(a.sh + s));
         }
+        up_store(a, j, lv, up_cell(a, lv, f), make_uint2(f, c | OG_LEAF_BIT), M, ax, ay, az, lo, hi, hm);
     }
-    // (B) internal nodes, deepest level first
+    // (B) internal nodes, deepest level first: sums over the children in order, all records
     int max_lv = 0;
     for (int lv = 0; lv <= OG_MAX_LEVEL; ++lv)
         if (a.level_start[lv + 1] > a.level_start[lv]) max_lv = lv;
@@ -322,31 +344,8 @@ k_upward(UpArgs a)
                 hi.x = fmaxf(hi.x, h4.x); hi.y = fmaxf(hi.y, h4.y); hi.z = fmaxf(hi.z, h4.z);
                 hm = fmaxf(hm, l4.w);
             }
-            up_store(a, j, M, ax, ay, az, lo, hi, hm);
+            up_store(a, j, lv, up_cell(a, lv, a.first[j]), make_uint2(fc, nc), M, ax, ay, az, lo, hi, hm);
         }
-    }
-    // (C) packed walk records n1, n2 (og_internal.cuh) from the finished fp32 records.  R and ng are
-    // bounds used only by conservative tests of the walk, so they are rounded up.
-    grid.sync();
-    for (uint32_t j = t0; j < n_nodes; j += stride) {
-        const float4 s = __ldcg(a.com + j), cc = __ldcg(a.cell + j), lo = __ldcg(a.lo + j), hi = __ldcg(a.hi + j);
-        const uint2 info = __ldcg(a.info + j);
-        const double ex = fmax((double)s.x - (double)lo.x, (double)hi.x - (double)s.x),
-                     ey = fmax((double)s.y - (double)lo.y, (double)hi.y - (double)s.y),
-                     ez = fmax((double)s.z - (double)lo.z, (double)hi.z - (double)s.z);
-        const float R = __double2float_ru(sqrt(ex * ex + ey * ey + ez * ez) * (1.0 + 1e-6));
-        const double lim = 0.6 * (double)cc.w;
-        const double gx = lim + fabs((double)s.x - (double)cc.x), gy = lim + fabs((double)s.y - (double)cc.y),
-                     gz = lim + fabs((double)s.z - (double)cc.z);
-        const float rg = __double2float_ru(sqrt(gx * gx + gy * gy + gz * gz) * (1.0 + 1e-6));
-        const uint32_t leaf = (info.y & OG_LEAF_BIT) ? 1u : 0u;
-        const uint32_t cnt = info.y & ~OG_LEAF_BIT;
-        if (cnt >= (1u << 26)) atomicOr(a.status, OG_DEV_NODE_OVERFLOW);   // does not fit the packed record
-        const uint32_t meta = ((uint32_t)a.level[j] << 27) | (leaf << 26) | (cnt & 0x03ffffffu);
-        uint4 *r = a.rec + 3 * (size_t)j;
-        r[0] = make_uint4(__float_as_uint(s.x), __float_as_uint(s.y), __float_as_uint(s.z), __float_as_uint(s.w));
-        r[1] = make_uint4(__float_as_uint(R), __float_as_uint(fmaxf(rg, lo.w)), info.x, meta);
-        r[2] = make_uint4(__float_as_uint(cc.x), __float_as_uint(cc.y), __float_as_uint(cc.z), __float_as_uint(lo.w));
     }
 }
 

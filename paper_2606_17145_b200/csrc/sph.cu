@@ -4,8 +4,9 @@
 // target particle and processes them in a separate evaluate function").  Readings R43..R47, DESIGN.md Sec. 12.
 //
 // k_sph_density: one warp per target.
-//   1. radius H: the caller's h_guess, or the half side of the deepest ancestor of the target that still holds
-//      n_des particles (found by descending the target's own path from the root);
+//   1. radius H: 1.05 x the caller's h_guess, or from the deepest ancestor cell of the target that still holds n_des
+//      particles (found by descending the target's own path from the root): the radius that would hold 1.5 n_des
+//      at the cell's mean density;
 //   2. COLLECT: the warp walks the tree (32 nodes per step from a warp-private stack in shared memory; a node is
 //      opened when the nearest image of its tight AABB is within H of the target; children are contiguous) and
 //      appends (r, m) of every particle with r < H to a candidate list in shared memory (ballot compaction);
@@ -198,11 +199,12 @@ __global__ void __launch_bounds__(SPH_WARPS * 32) k_sph_density(const __grid_con
         const float4 p = __ldg(a.spos + slot);
         float H;
         if (a.h_guess) {
-            H = __ldg(a.h_guess + out);
+            H = 1.05f * __ldg(a.h_guess + out);     // (a previous h: N(H) >= n_des at the first try, almost always)
             if (!(H > 0.0f)) H = 1.0e-3f * a.L;
         } else {
-            // deepest ancestor of the target with at least n_des particles (the root if there is none)
-            uint32_t node = 0u, level = 0u;
+            // deepest ancestor of the target with at least n_des particles (the root if there is none): its particle
+            // count and side give the local density, hence the radius of a sphere that holds about 1.5 n_des
+            uint32_t node = 0u, level = 0u, ncount = a.n;
             for (;;) {
                 const uint32_t nc = __ldg(a.nchild + node);
                 if (nc == 0u) break;
@@ -214,9 +216,10 @@ __global__ void __launch_bounds__(SPH_WARPS * 32) k_sph_density(const __grid_con
                 const int src = __ffs(mine) - 1;
                 const uint32_t ccnt = __shfl_sync(0xffffffffu, cc, src);
                 if ((float)ccnt < a.n_des) break;
-                node = fc + (uint32_t)src; ++level;
+                node = fc + (uint32_t)src; ncount = ccnt; ++level;
             }
-            H = 0.5f * a.L * __uint_as_float((127u - level) << 23);
+            const float l = a.L * __uint_as_float((127u - level) << 23);
+            H = l * cbrtf(0.358f * a.n_des / (float)ncount);
         }
         const float hcap = 0.5f * a.L * (1.0f - 1.0e-6f);
         H = fminf(H, hcap);

@@ -75,6 +75,22 @@ def test_argument_errors_and_no_cpu_fallback(B):
     assert B._lib.og_shortrange_accel(None, None, 0, None, None, None, None) == B.OG_ERR_INVALID_ARG
 
 
+def test_new_rows_reject_bad_arguments_without_a_device(B):
+    """Rows f3 / f4: NULL handles and out-of-range scalars are refused on the host before anything is enqueued."""
+    L = B._lib
+    assert L.og_sph_density(None, None, 10, C.c_float(32.0), C.c_float(0.0), None, None, None, None, None) == B.OG_ERR_INVALID_ARG
+    assert b"tree is NULL" in L.og_last_error()
+    assert L.og_shortrange_accel_ext(None, None, None, 10, None, None, None, None) == B.OG_ERR_INVALID_ARG
+    assert L.og_domain_cell_hist(None, 10, C.c_float(1.0), None, None) == B.OG_ERR_INVALID_ARG
+    assert L.og_domain_owner(None, 10, C.c_float(1.0), None, 4, None, None) == B.OG_ERR_INVALID_ARG
+    cnt = C.c_uint64(7)
+    assert L.og_let_export_list(None, 0, None, 0, C.c_float(0.1), C.c_float(1.0), None, C.byref(cnt), None) == B.OG_OK
+    assert cnt.value == 0                                                   # empty input: a no-op that reports 0
+    assert L.og_let_export_list(None, 5, None, 3, C.c_float(0.1), C.c_float(1.0), None, C.byref(cnt), None) == B.OG_ERR_INVALID_ARG
+    assert L.og_let_accumulate(None, None, None, None, None, 5, 5, None) == B.OG_ERR_INVALID_ARG
+    assert L.og_let_accumulate(None, None, None, None, None, 0, 5, None) == B.OG_OK
+
+
 def test_product_does_not_import_oracle():
     pkg = os.path.join(ROOT, "paper_2606_17145_b200")
     for dirpath, _, files in os.walk(pkg):
