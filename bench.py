@@ -39,7 +39,7 @@ from paper_2606_17145_b200 import workloads as W  # noqa: E402
 METRIC = "short-range tree-gravity particles/s (tree build + walk, 1 step) on B200"
 UNIT = "particles/s"
 SM_LANES = 128          # FP32 lanes per SM (B200)
-KERNELS_PER_BUILD = 1 + 8 * 3 + 1 + 2   # keys, 8 x (hist, scan, scatter), gather, octree + upward
+KERNELS_PER_BUILD = 1 + (2 + 8) + 1 + 2   # keys, sort (digit histograms, their scan, 8 one-sweep passes), gather, octree + upward
 KERNELS_PER_WALK_ALL = 1
 
 
@@ -446,10 +446,10 @@ def run_ours(args):
         "clocks": clocks,
         "e2e": {"value": aggregate(n_act_all, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e, "steps": e2e_steps},
-        # with an explicit active list: slot keys, a radix sort of ceil(log2 n / 8) passes x 3 kernels, slot unpack, and
+        # with an explicit active list: slot keys, a radix sort (2 + ceil(log2 n / 8) one-sweep passes), slot unpack, and
         # the second instantiation of the walk kernel (the one the device-side decision does not pick returns at once)
         "gpu_launches": args.steps * (KERNELS_PER_BUILD + KERNELS_PER_WALK_ALL +
-                                      (0 if act is None else 2 + 3 * ((max(1, (n - 1).bit_length()) + 7) // 8) + 1)),
+                                      (0 if act is None else 2 + 2 + ((max(1, (n - 1).bit_length()) + 7) // 8) + 1)),
         "roofline": roofline,
         "breakdown_ms": {"build_a1_a5": ms_build, "walk_a6_a7": ms_walk},
         "particles_per_s_walk_only": na / (ms_walk * 1e-3),
