@@ -281,8 +281,9 @@ int og_ts_kick(float *vel, uint8_t *bin, float *a_old, const uint32_t *active_id
  *   tree       a tree from og_tree_build (its particles are the SPH particles; masses from the tree)
  *   active_idx DEVICE u32 [n_active] ORIGINAL indices of the targets, or NULL -> all n in identity order
  *   n_des      32/3 < n_des <= 256 (N(h) -> 32/3 as h -> 0 for an isolated particle)
- *   h_guess    DEVICE f32 [n_active] starting radius per target in active order (e.g. the previous step's h), or
- *              NULL -> derived from the tree (half the side of the deepest ancestor cell holding n_des particles)
+ *   h_guess    DEVICE f32 [n_active] an estimate of h per target in active order (e.g. the previous step's h; the search
+ *              starts at 1.05 x this; any positive value reaches the same root), or NULL -> derived from the tree (the
+ *              radius that holds 1.5 n_des at the mean density of the deepest ancestor cell with n_des particles)
  *   h_out      DEVICE f32 [n_active]; rho_out, nn_out (N at the returned h): DEVICE f32 [n_active] or NULL
  * Enqueues on `stream` (ordered after the tree's build).  Neighbour candidates are kept in a per-warp list of 1024
  * entries; a target whose root sphere holds more (a void particle whose kernel rim grazes a dense clump) is solved
