@@ -162,11 +162,25 @@ def let_forces(B, doms: dict, ex, box: float, prm, geometric: bool = False, want
     trees, boxes, acc, pot, tpos, teps, info = {}, {}, {}, {}, {}, {}, {"n_exported": {}}
     for r in ex.ranks:                                        # R50 + primary walk (home domain, self excluded)
         d = doms[r]
+        dev = d.pos.device
+        na = 0 if d.active is None else int(d.active.shape[0])
+        if d.pos.shape[0] == 0:                               # an empty domain owns no tree: nothing is exported to it
+            trees[r] = None
+            boxes[r] = torch.empty((0, 6), dtype=torch.float32, device=dev)
+            acc[r] = torch.zeros((0, 3), dtype=torch.float32, device=dev)
+            pot[r] = torch.zeros(0, dtype=torch.float32, device=dev) if want_pot else None
+            tpos[r] = torch.empty((0, 3), dtype=torch.float32, device=dev)
+            teps[r] = torch.empty(0, dtype=torch.float32, device=dev)
+            continue
         trees[r] = B.og_tree_build(d.pos, d.mass, d.eps, box, prm)
         mark("build")
         boxes[r] = top_boxes(B, trees[r])
         a_old = None if geometric else d.a_old
-        acc[r], pot[r] = B.og_shortrange_accel(trees[r], d.active, a_old, want_pot=want_pot)
+        if na:
+            acc[r], pot[r] = B.og_shortrange_accel(trees[r], d.active, a_old, want_pot=want_pot)
+        else:
+            acc[r] = torch.zeros((0, 3), dtype=torch.float32, device=dev)
+            pot[r] = torch.zeros(0, dtype=torch.float32, device=dev) if want_pot else None
         mark("primary_walk")
         al = d.active.long()
         tpos[r], teps[r] = d.pos[al].contiguous(), d.eps[al].contiguous()
@@ -177,7 +191,7 @@ def let_forces(B, doms: dict, ex, box: float, prm, geometric: bool = False, want
         ao = torch.zeros(tpos[r].shape[0], device=tpos[r].device) if (geometric or d.a_old is None) else d.a_old
         lists[r], send[r] = [], []
         for q in range(ex.R):
-            if q == r or all_boxes[q].shape[0] == 0:
+            if q == r or all_boxes[q].shape[0] == 0 or tpos[r].shape[0] == 0:
                 lst = torch.empty(0, dtype=torch.int32, device=tpos[r].device)
             else:
                 lst = B.og_let_export_list(tpos[r], all_boxes[q].to(tpos[r].device), r_cut, box)
@@ -192,7 +206,7 @@ def let_forces(B, doms: dict, ex, box: float, prm, geometric: bool = False, want
     for r in ex.ranks:                                        # secondary walk: all imported targets in one call
         cnt = [x.shape[0] for x in recv[r]]
         rows = torch.cat(recv[r], 0)
-        if rows.shape[0]:
+        if rows.shape[0] and trees[r] is not None:
             a, p = B.og_shortrange_accel_ext(trees[r], rows[:, 0:3].contiguous(), rows[:, 3].contiguous(),
                                              None if geometric else rows[:, 4].contiguous(), want_pot=want_pot)
             res = torch.cat([a, p[:, None] if want_pot else torch.zeros_like(a[:, :1])], 1)
@@ -210,9 +224,10 @@ def let_forces(B, doms: dict, ex, box: float, prm, geometric: bool = False, want
                 B.og_let_accumulate(acc[r], pot[r] if want_pot else None, lists[r][q], part[:, 0:3].contiguous(),
                                     part[:, 3].contiguous() if want_pot else None)
         out[r] = (acc[r], pot[r])
-        if B.og_tree_status(trees[r]) != B.OG_OK:
-            raise B.OgError(B.og_tree_status(trees[r]), B.og_last_error())
-        B.og_tree_free(trees[r])
+        if trees[r] is not None:
+            if B.og_tree_status(trees[r]) != B.OG_OK:
+                raise B.OgError(B.og_tree_status(trees[r]), B.og_last_error())
+            B.og_tree_free(trees[r])
     mark("sum")
     if timings is not None:
         torch.cuda.synchronize()

@@ -134,3 +134,72 @@ def test_let_pipeline_matches_oracle(B, name, R):
     assert oinfo["n_exported"].sum() <= n_exp <= oinfo["n_exported"].sum() * 1.001 + 2     # (the kernel's 1e-5 band)
     print(f"{name} R={R}: LET acc p99 {q99:.2e} max {mx:.2e}; pot p99 {np.percentile(ep, 99):.2e}; exported {n_exp} "
           f"target copies for {len(act)} targets")
+
+
+def test_let_empty_domains_active_subset_geometric_on_device(B):
+    """As tests/test_let_dist.py::test_empty_domains_..., through the kernels: 7 domains over three occupied cells."""
+    import torch
+    from paper_2606_17145_b200 import let
+    rng = np.random.default_rng(12)
+    L = 10.0
+    centres = np.array([[1.1, 1.1, 1.1], [1.3, 1.1, 1.1], [7.7, 3.3, 9.1]])
+    pos = np.vstack([c + rng.random((40, 3)) * 0.05 for c in centres]).astype(np.float32)
+    n = pos.shape[0]
+    mass = (rng.random(n) + 0.5).astype(np.float32)
+    eps = np.full(n, 1e-3, np.float32)
+    prm_o = oracle.make_params(L, 0.2, alpha=0.005, theta=0.5, leaf_max=4)
+    prm = B.make_params(0.2, alpha=0.005, theta=0.5, leaf_max=4)
+    R = 7
+    act = np.sort(rng.choice(n, 50, replace=False)).astype(np.uint32)
+    mask = np.zeros(n, bool); mask[act] = True
+    ex = let.LocalExchange(R)
+    parts = {}
+    for r in range(R):
+        sel = np.arange(r, n, R)
+        parts[r] = let.Domain(*(torch.from_numpy(x[sel]).cuda() for x in (pos, mass, eps)),
+                              torch.from_numpy(sel.astype(np.int64)).cuda(), torch.from_numpy(mask[sel]).cuda(), None)
+    doms, S = let.decompose(B, parts, ex, L)
+    assert [int(doms[r].pos.shape[0]) for r in range(R)].count(0) >= 3
+    res, info = let.let_forces(B, doms, ex, L, prm, geometric=True)
+    a_ref, p_ref, oinfo = olet.let_walk(pos, mass, eps, prm_o, R, active_idx=act, a_old=None)
+    assert np.array_equal(S, oinfo["splitters"])
+    got = np.zeros((n, 3)); gp = np.zeros(n)
+    for r in range(R):
+        g = doms[r].gid[doms[r].active.long()].cpu().numpy()
+        got[g] = res[r][0].cpu().numpy(); gp[g] = res[r][1].cpu().numpy()
+    check_acc(got[act], a_ref, what="LET with empty domains")
+    ep = rel_err_scalar(gp[act], p_ref)
+    assert np.percentile(ep, 99) <= 1e-4 and ep.max() <= 1e-2
+
+
+def test_external_targets_on_top_of_tree_particles_and_across_the_wall(B):
+    """External targets that coincide with particles of the tree (r = 0 pairs: force 0, potential -(14/5) G m / h, C5;
+    nothing is excluded) and targets within r_cut of the periodic wall."""
+    import torch
+    w = W.make("uniform32", small=True)
+    rng = np.random.default_rng(3)
+    k = rng.choice(w.n, 300, replace=False)
+    wall = rng.random((300, 3)).astype(np.float32) * w.L
+    wall[:, 0] = (rng.random(300) * 0.5 * w.r_s).astype(np.float32)             # hugging x = 0
+    wall[150:, 1] = np.float32(w.L) - (rng.random(150) * 0.5 * w.r_s).astype(np.float32)
+    wall[wall >= w.L] = 0.0
+    tpos = np.vstack([w.pos[k], wall]).astype(np.float32)
+    teps = np.full(600, float(w.eps[0]), np.float32)
+    pos, mass, eps = to_dev(w)
+    tree = B.og_tree_build(pos, mass, eps, w.L, gpu_params(w))
+    ot = oracle.build_tree(w.pos, w.mass, w.eps, oracle_params(w))
+    th = oracle.particle_h(teps)
+    ao_g, _, _ = oracle.walk_ext(ot, tpos, th, None)
+    a_old = np.linalg.norm(ao_g, axis=1).astype(np.float32)
+    ao, po, _ = oracle.walk_ext(ot, tpos, th, a_old)
+    a, p = B.og_shortrange_accel_ext(tree, torch.from_numpy(tpos).cuda(), torch.from_numpy(teps).cuda(),
+                                     torch.from_numpy(a_old).cuda())
+    check_acc(a.cpu().numpy(), ao, what="ext coincident / wall")
+    ep = rel_err_scalar(p.cpu().numpy(), po)
+    assert np.percentile(ep, 99) <= 1e-4 and ep.max() <= 1e-2
+    # the coincident pair really is in the sum: the potential of such a target is lower than without its twin
+    d, pd = oracle.direct_ext(np.delete(w.pos, k[:1], 0), np.delete(w.mass, k[:1]), np.delete(w.eps, k[:1]), oracle_params(w),
+                              tpos[:1], teps[:1])
+    assert po[0] < pd[0]
+    assert B.og_tree_status(tree) == B.OG_OK
+    B.og_tree_free(tree)

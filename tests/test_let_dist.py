@@ -102,3 +102,45 @@ def test_world2_gloo_pipeline_equals_local_emulation_and_oracle():
         seen += len(k)
     assert seen == len(act)
     assert 0 < oinfo["n_exported"].sum() < len(act)                                       # some, not all, are exported
+
+
+def test_empty_domains_and_active_subset_local_emulation():
+    """More domains than occupied level-5 cells: some domains own nothing (no tree, nothing exported to them); a sparse
+    active subset; geometric criterion.  One process, oracle-backed stand-in, against oracle.let."""
+    import torch
+    import let_stub
+    import oracle
+    from oracle import let as olet
+    from paper_2606_17145_b200 import let
+    rng = np.random.default_rng(12)
+    L = 10.0
+    # three tight clumps: three occupied level-5 cells (side L / 32), 7 domains
+    centres = np.array([[1.1, 1.1, 1.1], [1.3, 1.1, 1.1], [7.7, 3.3, 9.1]])
+    pos = np.vstack([c + rng.random((40, 3)) * 0.05 for c in centres]).astype(np.float32)
+    n = pos.shape[0]
+    mass = (rng.random(n) + 0.5).astype(np.float32)
+    eps = np.full(n, 1e-3, np.float32)
+    prm = oracle.make_params(L, 0.2, alpha=0.005, theta=0.5, leaf_max=4)
+    R = 7
+    act = np.sort(rng.choice(n, 50, replace=False)).astype(np.uint32)
+    mask = np.zeros(n, bool); mask[act] = True
+    ex = let.LocalExchange(R)
+    parts = {}
+    for r in range(R):
+        sel = np.arange(r, n, R)
+        parts[r] = let.Domain(torch.from_numpy(pos[sel]), torch.from_numpy(mass[sel]), torch.from_numpy(eps[sel]),
+                              torch.from_numpy(sel.astype(np.int64)), torch.from_numpy(mask[sel]), None)
+    doms, S = let.decompose(let_stub, parts, ex, L)
+    sizes = [int(doms[r].pos.shape[0]) for r in range(R)]
+    assert sum(sizes) == n and sizes.count(0) >= 3                       # empty domains exist
+    res, info = let.let_forces(let_stub, doms, ex, L, prm, geometric=True)
+    a_ref, p_ref, oinfo = olet.let_walk(pos, mass, eps, prm, R, active_idx=act, a_old=None)
+    assert np.array_equal(S, oinfo["splitters"])
+    got = np.zeros((n, 3)); gp = np.zeros(n); seen = np.zeros(n, bool)
+    for r in range(R):
+        g = doms[r].gid[doms[r].active.long()].numpy()
+        got[g] = res[r][0].numpy(); gp[g] = res[r][1].numpy(); seen[g] = True
+    assert np.array_equal(np.flatnonzero(seen), act)
+    assert np.abs(got[act] - a_ref).max() <= 1e-5 * np.abs(a_ref).max()
+    assert np.abs(gp[act] - p_ref).max() <= 1e-5 * np.abs(p_ref).max()
+    assert sum(info["n_exported"].values()) == int(oinfo["n_exported"].sum()) > 0
