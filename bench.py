@@ -710,6 +710,24 @@ def run_pm(args):
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / args.steps
+    # the same particles in the tree's (Morton) order, as a code that keeps its particles along a space-filling curve
+    # passes them: the mass assignment then sums the runs of particles that share a grid point inside the warp
+    prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8)
+    tree = B.og_tree_build(pos, mass, torch.from_numpy(w.eps).to(dev), w.L, prm)
+    perm = B.og_tree_get(tree, B.OG_F_PERM).long()
+    pos_s, mass_s = pos[perm].contiguous(), mass[perm].contiguous()
+    B.og_tree_free(tree)
+    for _ in range(max(args.warmup, 1)):
+        acc_s, pot_s = B.og_pm_longrange(pm, pos_s, mass_s)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        acc_s, pot_s = B.og_pm_longrange(pm, pos_s, mass_s)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_sorted = e0.elapsed_time(e1) / args.steps
+    arms = float(torch.sqrt((acc * acc).sum(1).mean()).item())
+    diff_sorted = float((acc_s - acc[perm]).abs().max().item()) / arms
     peaks, src = measured_peaks()
     g = float(ng) ** 3
     # deposit: 16 B in per particle + the mass grid written once; R2C + C2R: each grid read and written once per FFT
@@ -719,10 +737,13 @@ def run_pm(args):
     hbm = peaks.get("hbm_gbs", 0.0)
     line = {"mode": "pm_longrange", "metric": "PM long-range force particles/s (CIC deposit + cuFFT + Green + gradient + CIC "
             "interpolation) on B200", "value": w.n / (ms * 1e-3), "unit": "particles/s", "n_gpus": 1, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+            "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_morton_ordered_input": ms_sorted,
+            "value_morton_ordered_input": w.n / (ms_sorted * 1e-3), "max_abs_acc_difference_between_the_orders_over_rms": diff_sorted,
+            "higher_is_better": True, "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "n": w.n, "ng": ng, "r_s": w.r_s, "box": w.L},
             "roofline": {"bound": "hbm", "achieved": bytes_alg / (ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
                          "frac": (bytes_alg / (ms * 1e-3) / 1e9 / hbm) if hbm else None, "traffic": None,
+                         "frac_morton_ordered_input": (bytes_alg / (ms_sorted * 1e-3) / 1e9 / hbm) if hbm else None,
                          "algorithmic_bytes": bytes_alg, "peak_source": src},
             "checksum_mean_abs_acc": float(acc.abs().mean().item())}
     B.og_pm_free(pm)

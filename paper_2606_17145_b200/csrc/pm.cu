@@ -34,15 +34,21 @@ namespace {
 
 __device__ __forceinline__ uint32_t wrap_idx(int i, int ng) { return (uint32_t)(i < 0 ? i + ng : (i >= ng ? i - ng : i)); }
 
-// R31.  One thread per particle, 8 red.global.add.f32.
+// R31.  One thread per particle.  Particles that are neighbours in the input and share their base grid point (the usual
+// case when the caller keeps its particles in space-filling-curve order, as a tree code does: the points of a 2^k mesh
+// are octree cells, so such particles are consecutive) are summed inside the warp first -- a segmented scan over the
+// runs of equal base points, eight weights at once -- and only the last lane of a run issues the 8 red.global.add.f32;
+// unordered input (no runs) skips the scan.
 __global__ void __launch_bounds__(256)
 k_pm_deposit(const float *__restrict__ pos, const float *__restrict__ mass, uint64_t n, float inv_delta, int ng,
              float *__restrict__ mgrid)
 {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const float x = __ldg(pos + 3 * i) * inv_delta, y = __ldg(pos + 3 * i + 1) * inv_delta, z = __ldg(pos + 3 * i + 2) * inv_delta;
-    const float m = __ldg(mass + i);
+    const uint32_t lane = threadIdx.x & 31u;
+    const bool ok = i < n;
+    const uint64_t ii = ok ? i : n - 1;
+    const float x = __ldg(pos + 3 * ii) * inv_delta, y = __ldg(pos + 3 * ii + 1) * inv_delta, z = __ldg(pos + 3 * ii + 2) * inv_delta;
+    const float m = ok ? __ldg(mass + ii) : 0.0f;
     const float fx0 = floorf(x), fy0 = floorf(y), fz0 = floorf(z);
     const float fx = x - fx0, fy = y - fy0, fz = z - fz0;
     int ix = (int)fx0, iy = (int)fy0, iz = (int)fz0;
@@ -51,13 +57,39 @@ k_pm_deposit(const float *__restrict__ pos, const float *__restrict__ mass, uint
                    z0 = wrap_idx(iz, ng), z1 = wrap_idx(iz + 1, ng);
     const float wx[2] = {1.0f - fx, fx}, wy[2] = {1.0f - fy, fy}, wz[2] = {1.0f - fz, fz};
     const uint32_t xs[2] = {x0, x1}, ys[2] = {y0, y1}, zs[2] = {z0, z1};
+    float v[8];
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll
         for (int b = 0; b < 2; ++b)
 #pragma unroll
-            for (int c = 0; c < 2; ++c)
-                atomicAdd(mgrid + ((size_t)xs[a] * ng + ys[b]) * ng + zs[c], m * wx[a] * wy[b] * wz[c]);
+            for (int c = 0; c < 2; ++c) v[4 * a + 2 * b + c] = m * wx[a] * wy[b] * wz[c];
+    const uint32_t base = ok ? (x0 * (uint32_t)ng + y0) * (uint32_t)ng + z0 : 0xffffffffu;
+    const uint32_t prev = __shfl_up_sync(0xffffffffu, base, 1);
+    const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0u || base != prev);
+    if (heads != 0xffffffffu) {
+        // inclusive segmented scan over the runs; my_head = the lane that starts this lane's run
+        const uint32_t my_head = 31u - (uint32_t)__clz(heads & (0xffffffffu >> (31u - lane)));
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const bool take = lane >= my_head + (uint32_t)o;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const float up = __shfl_up_sync(0xffffffffu, v[c], o);
+                if (take) v[c] += up;
+            }
+        }
+    }
+    const bool tail = lane == 31u || ((heads >> (lane + 1u)) & 1u);
+    if (ok && tail) {
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int b = 0; b < 2; ++b)
+#pragma unroll
+                for (int c = 0; c < 2; ++c)
+                    atomicAdd(mgrid + ((size_t)xs[a] * ng + ys[b]) * ng + zs[c], v[4 * a + 2 * b + c]);
+    }
 }
 
 // R32.  One thread per complex element of the half spectrum [ng][ng][ng/2 + 1].
