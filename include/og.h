@@ -120,7 +120,8 @@ typedef enum {
     OG_F_LEVEL_START = 14,  /* u32 [23]    node index where each level starts (BFS)        */
     OG_F_WALK_COST = 15     /* u32 [n]     OG_COUNT trees only: interactions (accepted nodes + particle pairs)
                                evaluated for each target of the LAST walk, in the caller's active order (the first
-                               n_active entries); the per-target work figure a host code balances its next step by */
+                               n_active entries); the per-target work figure a host code balances its next step by
+                               (not written by a walk of more than n targets or of external targets)              */
 } og_field;
 
 /* Bytes of DEVICE workspace og_tree_build needs for n particles (0 on invalid input).    */

@@ -1031,7 +1031,9 @@ cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t 
     a.status = t->d_status;
     a.counters = t->d_counters;
     a.spill = reinterpret_cast<uint32_t *>(t->walk_spill);
-    a.cost = t->walk_cost;
+    // the per-target work array has one entry per particle of the tree: not written for external targets, nor for a
+    // list longer than that (duplicates)
+    a.cost = (ext == nullptr && n_active <= t->n) ? t->walk_cost : nullptr;
     a.spill_cap = t->walk_spill_cap;
     a.stack_cap = t->prm.walk_stack_entries ? min(t->prm.walk_stack_entries, (uint32_t)GW_STACK) : (uint32_t)GW_STACK;
     const og_params &p = t->prm;

@@ -203,3 +203,15 @@ def test_external_targets_on_top_of_tree_particles_and_across_the_wall(B):
     assert po[0] < pd[0]
     assert B.og_tree_status(tree) == B.OG_OK
     B.og_tree_free(tree)
+    # a counting tree (OG_COUNT) and MORE external targets than the tree has particles: same numbers, nothing overrun
+    small = W.Workload("few", w.pos[:200].copy(), w.mass[:200].copy(), w.eps[:200].copy(), w.L, w.r_s)
+    tc = B.og_tree_build(*(torch.from_numpy(x).cuda() for x in (small.pos, small.mass, small.eps)), small.L,
+                         gpu_params(small, flags=B.OG_COUNT))
+    guard = torch.full((4096,), 7.0, device="cuda")                              # allocated right after the tree
+    a2, p2 = B.og_shortrange_accel_ext(tc, torch.from_numpy(tpos).cuda(), torch.from_numpy(teps).cuda(), None)
+    oc = oracle.build_tree(small.pos, small.mass, small.eps, oracle_params(small))
+    ao2, po2, _ = oracle.walk_ext(oc, tpos, th, None)
+    nz = np.linalg.norm(ao2, axis=1) > 0
+    check_acc(a2.cpu().numpy()[nz], ao2[nz], what="ext on a counting tree")
+    assert B.og_tree_status(tc) == B.OG_OK and float(guard.min()) == 7.0
+    B.og_tree_free(tc)
