@@ -73,6 +73,26 @@ def test_splitters_hand_built():
     assert let.splitters(np.zeros(let.N_CELLS, np.int64), 3).tolist() == [0, 0, 0, 32768]
 
 
+def test_splitters_equal_the_oracle_rule_on_random_histograms():
+    """paper_2606_17145_b200/let.py and oracle/let.py state R49 independently (searchsorted vs an explicit scan)."""
+    from oracle import let as olet
+    from paper_2606_17145_b200 import let
+    rng = np.random.default_rng(77)
+    for trial in range(40):
+        h = np.zeros(let.N_CELLS, np.int64)
+        k = int(rng.integers(1, 4000))
+        cells = rng.choice(let.N_CELLS, size=k, replace=False)
+        h[cells] = rng.integers(1, 10 ** int(rng.integers(1, 6)), size=k)
+        for R in (1, 2, 3, 5, 8, 16, 64):
+            S = let.splitters(h, R)
+            assert np.array_equal(S, olet.splitters(h, R)), (trial, R)
+            assert S[0] == 0 and S[-1] == let.N_CELLS and np.all(np.diff(S) >= 0)
+            # balance: no domain exceeds its share by more than the largest cell
+            per = np.add.reduceat(np.r_[h, 0], np.minimum(S[:-1], let.N_CELLS))[:R] * (np.diff(S) > 0)
+            assert per.sum() == h.sum()
+            assert per.max() <= -(-h.sum() // R) + h.max()
+
+
 def test_world2_gloo_pipeline_equals_local_emulation_and_oracle():
     import torch.multiprocessing as mp
     import oracle
