@@ -21,8 +21,8 @@
 namespace {
 
 constexpr int SPH_WARPS = 4;
-constexpr int SPH_CAP = 1024;    // candidates per warp
-constexpr int SPH_QCAP = 512;    // pending nodes per warp
+constexpr int SPH_CAP = 512;     // candidates per warp
+constexpr int SPH_QCAP = 256;    // pending nodes per warp
 
 struct __align__(16) SphSmem {
     float cr[SPH_CAP];           // distance to the target

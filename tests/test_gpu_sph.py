@@ -169,7 +169,7 @@ def test_sph_rim_grazing_a_dense_clump_takes_the_streaming_path(B):
     t = np.concatenate([np.arange(0, 6000, 40), np.arange(6000, n)])
     _compare(w, t, h.cpu().numpy().astype(np.float64), rho.cpu().numpy().astype(np.float64),
              nn.cpu().numpy().astype(np.float64), 64.0, "rim")
-    # the void targets do need more than 1024 candidates
+    # the void targets do need more candidates than the per-warp list holds (512)
     d = np.linalg.norm(w.pos[:6000].astype(np.float64) - w.pos[6000].astype(np.float64), axis=1)
     assert (d < float(h[6000])).sum() > 1024
     B.og_tree_free(tree)
