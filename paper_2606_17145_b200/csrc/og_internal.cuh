@@ -69,7 +69,7 @@ struct og_tree {
     uint4 *node_rec;           // [3 n_nodes]: n0, n1, n2 of node j at 3 j, 3 j + 1, 3 j + 2 (48 contiguous bytes)
     // small device state
     uint32_t *d_level_start;   // [24]: start index per level, [22] = n_nodes, [23] = max level
-    uint32_t *d_status;        // [16]: [0] latched status bits, [1] walk work counter, [2] sparse-active-list flag
+    uint32_t *d_status;        // [16]: [0] latched status bits, [1] walk work counter, [2] sparse-active-list flag, [3] SPH ticket
     uint32_t *walk_cost;       // [n] OG_COUNT only: interactions evaluated per target of the last walk, caller's order
     unsigned long long *d_counters;  // [OGC_N]
     // walk scratch (spill stacks), allocated lazily

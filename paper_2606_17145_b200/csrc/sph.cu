@@ -43,6 +43,7 @@ struct SphArgs {
     uint32_t n, n_active;
     float L, invL, n_des, tol_n;
     uint32_t *status;
+    uint32_t *ticket;            // zeroed before the launch
 };
 
 __device__ __forceinline__ float sph_wrap(float d, float L, float invL) { return fmaf(-L, rintf(d * invL), d); }
@@ -186,8 +187,17 @@ __global__ void __launch_bounds__(SPH_WARPS * 32) k_sph_density(const __grid_con
     __shared__ SphSmem sm[SPH_WARPS];
     const uint32_t lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
     SphSmem &s = sm[wid];
-    const uint32_t nwarps = gridDim.x * SPH_WARPS;
-    for (uint32_t k = blockIdx.x * SPH_WARPS + wid; k < a.n_active; k += nwarps) {
+    // targets are handed out four at a time by a ticket: a few targets cost a thousand times the typical one (their
+    // kernel rim grazes a dense clump and every trial radius re-walks the tree), and with a fixed assignment the warps
+    // that drew them finished long after the others
+    uint32_t k = 0, kend = 0;
+    for (;; ++k) {
+        if (k >= kend) {
+            if (lane == 0) k = atomicAdd(a.ticket, 4u);
+            k = __shfl_sync(0xffffffffu, k, 0);
+            kend = min(k + 4u, a.n_active);
+            if (k >= a.n_active) break;
+        }
         uint32_t slot, out;
         if (a.active_idx) {
             const uint32_t i = __ldg(a.active_idx + k);
@@ -332,6 +342,9 @@ cudaError_t ogk_sph_density(const og_tree *t, const uint32_t *active_idx, uint64
     a.n = (uint32_t)t->n; a.n_active = (uint32_t)n_active;
     a.L = t->box; a.invL = 1.0f / t->box; a.n_des = n_des; a.tol_n = tol_n;
     a.status = t->d_status;
+    a.ticket = t->d_status + 3;
+    cudaError_t e0 = cudaMemsetAsync(a.ticket, 0, sizeof(uint32_t), st);
+    if (e0 != cudaSuccess) return e0;
     int per_sm = 0;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sph_density, SPH_WARPS * 32, 0);
     if (e != cudaSuccess) return e;
