@@ -131,7 +131,56 @@ __device__ int sph_scan(const SphArgs &a, SphSmem &s, float px, float py, float 
         if (qn + (int)total > qcap) return -1;
         for (uint32_t k = 0; k < nch; ++k) q[qn + (incl - nch) + k] = info.x + k;
         qn += (int)total;
-        uint32_t lb = __ballot_sync(0xffffffffu, hit && leaf);
+        // Opened leaves.  Every lane takes ITS OWN leaf (<= 32 particles; the few larger ones below) and tests its particles
+        // one after the other: the loads of all the leaves of the batch are in flight together (one L2 round trip per
+        // batch instead of one per leaf).  The list keeps the order leaf by leaf (ascending lane), particle by particle.
+        const bool small_leaf = hit && leaf && c <= 32u;
+        uint32_t inmask = 0u;
+        if (small_leaf) {
+            for (uint32_t j = 0; j < c; ++j) {
+                const float4 pq = __ldg(a.spos + info.x + j);
+                const float dx = sph_wrap(pq.x - px, a.L, a.invL), dy = sph_wrap(pq.y - py, a.L, a.invL),
+                            dz = sph_wrap(pq.z - pz, a.L, a.invL);
+                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                if (r2 < H2) {
+                    if (STORE) {
+                        inmask |= 1u << j;
+                    } else {
+                        float w, uwp;
+                        sph_w(sqrtf(r2) * hinv, w, uwp);
+                        sa += w; sb += uwp; sc = fmaf(pq.w, w, sc);
+                        ++inmask;                    // (a count in this mode)
+                    }
+                }
+            }
+        }
+        {
+            const uint32_t mine = STORE ? (uint32_t)__popc(inmask) : inmask;
+            uint32_t run = mine;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xffffffffu, run, o);
+                if (lane >= (uint32_t)o) run += y;
+            }
+            const uint32_t tot = __shfl_sync(0xffffffffu, run, 31);
+            if (STORE) {
+                if (cnt + (int)tot > SPH_CAP) return -1;
+                uint32_t at = (uint32_t)cnt + run - mine;
+                while (inmask) {
+                    const uint32_t j = (uint32_t)__ffs(inmask) - 1u;
+                    inmask &= inmask - 1u;
+                    const float4 pq = __ldg(a.spos + info.x + j);
+                    const float dx = sph_wrap(pq.x - px, a.L, a.invL), dy = sph_wrap(pq.y - py, a.L, a.invL),
+                                dz = sph_wrap(pq.z - pz, a.L, a.invL);
+                    s.cr[at] = sqrtf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+                    s.cm[at] = pq.w;
+                    ++at;
+                }
+            }
+            cnt += (int)tot;
+        }
+        // leaves with more than 32 particles (deepest level only): the warp takes them one by one, 32 particles at a time
+        uint32_t lb = __ballot_sync(0xffffffffu, hit && leaf && c > 32u);
         while (lb) {
             const int src = __ffs(lb) - 1;
             lb &= lb - 1u;
