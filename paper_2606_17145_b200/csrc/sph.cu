@@ -85,11 +85,18 @@ __device__ __forceinline__ void sph_number(const SphSmem &s, int cnt, float h, u
     hdN = -k * warp_sum(b);    // dN/dh = -(32/3) sum w'(u) u / h
 }
 
+// No periodic image can matter if the sphere (padded) lies inside [0, L) on every axis: the scans then skip the wraps.
+__device__ __forceinline__ bool sph_interior(const SphArgs &a, float px, float py, float pz, float H)
+{
+    const float e = H * (1.0f + 1.0e-5f) + 1.0e-6f * a.L;
+    return px - e >= 0.0f && py - e >= 0.0f && pz - e >= 0.0f && px + e < a.L && py + e < a.L && pz + e < a.L;
+}
+
 // Step 2.  STORE: fills the candidate list with every particle closer than H to (px, py, pz) and returns their number,
 // or -1 if the list or the node stack overflowed.  !STORE (the fallback of a target whose candidates do not fit the
 // list): nothing is stored, the lanes add w, u w' and m w of the particles inside H = h to (sa, sb, sc) on the fly, and
 // the node stack may use the whole per-warp area; -1 only if even that stack overflows.
-template <bool STORE>
+template <bool STORE, bool WRAP>
 __device__ int sph_scan(const SphArgs &a, SphSmem &s, float px, float py, float pz, float H, uint32_t lane, float &sa,
                         float &sb, float &sc)
 {
@@ -112,25 +119,17 @@ __device__ int sph_scan(const SphArgs &a, SphSmem &s, float px, float py, float 
             const uint32_t node = q[qn + lane];
             const float4 lo = __ldg(a.lo + node), hi = __ldg(a.hi + node);
             info = __ldg(a.info + node);
-            const float dx = fmaxf(fabsf(sph_wrap(0.5f * (lo.x + hi.x) - px, a.L, a.invL)) - (0.5f * (hi.x - lo.x) + pad), 0.0f);
-            const float dy = fmaxf(fabsf(sph_wrap(0.5f * (lo.y + hi.y) - py, a.L, a.invL)) - (0.5f * (hi.y - lo.y) + pad), 0.0f);
-            const float dz = fmaxf(fabsf(sph_wrap(0.5f * (lo.z + hi.z) - pz, a.L, a.invL)) - (0.5f * (hi.z - lo.z) + pad), 0.0f);
+            float cx = 0.5f * (lo.x + hi.x) - px, cy = 0.5f * (lo.y + hi.y) - py, cz = 0.5f * (lo.z + hi.z) - pz;
+            if (WRAP) { cx = sph_wrap(cx, a.L, a.invL); cy = sph_wrap(cy, a.L, a.invL); cz = sph_wrap(cz, a.L, a.invL); }
+            const float dx = fmaxf(fabsf(cx) - (0.5f * (hi.x - lo.x) + pad), 0.0f);
+            const float dy = fmaxf(fabsf(cy) - (0.5f * (hi.y - lo.y) + pad), 0.0f);
+            const float dz = fmaxf(fabsf(cz) - (0.5f * (hi.z - lo.z) + pad), 0.0f);
             hit = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) <= H2n;
         }
         __syncwarp();
         const bool leaf = (info.y & OG_LEAF_BIT) != 0u;
         const uint32_t c = info.y & ~OG_LEAF_BIT;
         const uint32_t nch = (hit && !leaf) ? c : 0u;
-        uint32_t incl = nch;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= (uint32_t)o) incl += y;
-        }
-        const uint32_t total = __shfl_sync(0xffffffffu, incl, 31);
-        if (qn + (int)total > qcap) return -1;
-        for (uint32_t k = 0; k < nch; ++k) q[qn + (incl - nch) + k] = info.x + k;
-        qn += (int)total;
         // Opened leaves.  Every lane takes ITS OWN leaf (<= 32 particles; the few larger ones below) and tests its particles
         // one after the other: the loads of all the leaves of the batch are in flight together (one L2 round trip per
         // batch instead of one per leaf).  The list keeps the order leaf by leaf (ascending lane), particle by particle.
@@ -139,8 +138,8 @@ __device__ int sph_scan(const SphArgs &a, SphSmem &s, float px, float py, float 
         if (small_leaf) {
             for (uint32_t j = 0; j < c; ++j) {
                 const float4 pq = __ldg(a.spos + info.x + j);
-                const float dx = sph_wrap(pq.x - px, a.L, a.invL), dy = sph_wrap(pq.y - py, a.L, a.invL),
-                            dz = sph_wrap(pq.z - pz, a.L, a.invL);
+                float dx = pq.x - px, dy = pq.y - py, dz = pq.z - pz;
+                if (WRAP) { dx = sph_wrap(dx, a.L, a.invL); dy = sph_wrap(dy, a.L, a.invL); dz = sph_wrap(dz, a.L, a.invL); }
                 const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
                 if (r2 < H2) {
                     if (STORE) {
@@ -154,31 +153,40 @@ __device__ int sph_scan(const SphArgs &a, SphSmem &s, float px, float py, float 
                 }
             }
         }
-        {
-            const uint32_t mine = STORE ? (uint32_t)__popc(inmask) : inmask;
-            uint32_t run = mine;
+        // one scan for both offsets: children pushed (high half, <= 8 x 32) and particles appended (low half, <= 32 x 32)
+        const uint32_t mine = STORE ? (uint32_t)__popc(inmask) : inmask;
+        const uint32_t both = (nch << 16) | mine;
+        uint32_t run = both;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t y = __shfl_up_sync(0xffffffffu, run, o);
-                if (lane >= (uint32_t)o) run += y;
-            }
-            const uint32_t tot = __shfl_sync(0xffffffffu, run, 31);
-            if (STORE) {
-                if (cnt + (int)tot > SPH_CAP) return -1;
-                uint32_t at = (uint32_t)cnt + run - mine;
-                while (inmask) {
-                    const uint32_t j = (uint32_t)__ffs(inmask) - 1u;
-                    inmask &= inmask - 1u;
-                    const float4 pq = __ldg(a.spos + info.x + j);
-                    const float dx = sph_wrap(pq.x - px, a.L, a.invL), dy = sph_wrap(pq.y - py, a.L, a.invL),
-                                dz = sph_wrap(pq.z - pz, a.L, a.invL);
-                    s.cr[at] = sqrtf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
-                    s.cm[at] = pq.w;
-                    ++at;
-                }
-            }
-            cnt += (int)tot;
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, run, o);
+            if (lane >= (uint32_t)o) run += y;
         }
+        const uint32_t tot2 = __shfl_sync(0xffffffffu, run, 31);
+        const uint32_t total = tot2 >> 16, tot = tot2 & 0xffffu;
+        if (qn + (int)total > qcap) return -1;
+        {
+            uint32_t *dst = q + qn + ((run - both) >> 16);
+#pragma unroll
+            for (uint32_t k = 0; k < 8u; ++k)
+                if (k < nch) dst[k] = info.x + k;
+        }
+        qn += (int)total;
+        if (STORE) {
+            if (cnt + (int)tot > SPH_CAP) return -1;
+            uint32_t at = (uint32_t)cnt + ((run - both) & 0xffffu);
+            while (inmask) {
+                const uint32_t j = (uint32_t)__ffs(inmask) - 1u;
+                inmask &= inmask - 1u;
+                const float4 pq = __ldg(a.spos + info.x + j);
+                float dx = pq.x - px, dy = pq.y - py, dz = pq.z - pz;
+                if (WRAP) { dx = sph_wrap(dx, a.L, a.invL); dy = sph_wrap(dy, a.L, a.invL); dz = sph_wrap(dz, a.L, a.invL); }
+                s.cr[at] = sqrtf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+                s.cm[at] = pq.w;
+                ++at;
+            }
+        }
+        cnt += (int)tot;
         // leaves with more than 32 particles (deepest level only): the warp takes them one by one, 32 particles at a time
         uint32_t lb = __ballot_sync(0xffffffffu, hit && leaf && c > 32u);
         while (lb) {
@@ -224,7 +232,8 @@ __device__ __forceinline__ bool sph_number_stream(const SphArgs &a, SphSmem &s, 
                                                   uint32_t lane, float &N, float &hdN, float &msum)
 {
     float sa = 0.0f, sb = 0.0f, sc = 0.0f;
-    const int cnt = sph_scan<false>(a, s, px, py, pz, h, lane, sa, sb, sc);
+    const int cnt = sph_interior(a, px, py, pz, h) ? sph_scan<false, false>(a, s, px, py, pz, h, lane, sa, sb, sc)
+                                                    : sph_scan<false, true>(a, s, px, py, pz, h, lane, sa, sb, sc);
     __syncwarp();
     const float k = 32.0f / 3.0f;
     N = k * warp_sum(sa); hdN = -k * warp_sum(sb); msum = warp_sum(sc);
@@ -288,7 +297,11 @@ __global__ void __launch_bounds__(SPH_WARPS * 32) k_sph_density(const __grid_con
         bool shrunk = false, regrown = false, fail = false;   // fail: pending nodes exceed even the fallback's stack
         float grow = 1.2599211f;
         for (int tries = 0; tries < 200; ++tries) {
-            { float d0 = 0.f, d1 = 0.f, d2 = 0.f; cnt = sph_scan<true>(a, s, p.x, p.y, p.z, H, lane, d0, d1, d2); }
+            {
+                float d0 = 0.f, d1 = 0.f, d2 = 0.f;
+                cnt = sph_interior(a, p.x, p.y, p.z, H) ? sph_scan<true, false>(a, s, p.x, p.y, p.z, H, lane, d0, d1, d2)
+                                                        : sph_scan<true, true>(a, s, p.x, p.y, p.z, H, lane, d0, d1, d2);
+            }
             __syncwarp();
             if (cnt < 0) {
                 if (regrown) break;            // no sphere both holds n_des and fits the list
