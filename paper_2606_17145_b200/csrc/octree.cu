@@ -349,6 +349,21 @@ k_upward(UpArgs a)
     }
 }
 
+// seed5[m] = the node that covers the level-5 cell with Morton index m: the node at level 5, or the leaf above it
+// (empty cells keep 0xffffffff).  One thread per node of the levels 0..5.
+__global__ void __launch_bounds__(256)
+k_seed5(const uint64_t *__restrict__ keys, const uint8_t *__restrict__ level, const uint32_t *__restrict__ first,
+        const uint8_t *__restrict__ nchild, const uint32_t *__restrict__ level_start, uint32_t *__restrict__ seed5)
+{
+    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= level_start[6]) return;
+    const uint32_t lv = level[j];
+    if (lv < 5u && nchild[j] != 0u) return;          // covered by its descendants
+    const uint32_t shift = 3u * (5u - lv);
+    const uint32_t m0 = ((uint32_t)(keys[first[j]] >> 48) >> shift) << shift;
+    for (uint32_t m = m0; m < m0 + (1u << shift); ++m) seed5[m] = j;
+}
+
 int coop_grid(const void *kernel, int threads, int sm_count)
 {
     int per_sm = 0;
@@ -389,5 +404,9 @@ cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st)
     e = cudaLaunchCooperativeKernel((const void *)k_upward,
                                     dim3(coop_grid((const void *)k_upward, OCT_THREADS, t->sm_count)),
                                     dim3(OCT_THREADS), args2, 0, st);
-    return e;
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(t->seed5, 0xff, 32768 * sizeof(uint32_t), st);
+    if (e != cudaSuccess) return e;
+    k_seed5<<<(37449 + 255) / 256, 256, 0, st>>>(t->keys, t->node_level, t->node_first, t->node_nchild, t->d_level_start, t->seed5);
+    return cudaGetLastError();
 }

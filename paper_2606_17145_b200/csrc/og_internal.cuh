@@ -70,6 +70,8 @@ struct og_tree {
     // small device state
     uint32_t *d_level_start;   // [24]: start index per level, [22] = n_nodes, [23] = max level
     uint32_t *d_status;        // [16]: [0] latched status bits, [1] walk work counter, [2] sparse-active-list flag, [3] SPH ticket
+    uint32_t *seed5;           // [32768] level-5 cell (Morton index) -> the node that covers it (at level 5, or the leaf above;
+                               // 0xffffffff: empty cell); entry points of the neighbour walk of og_sph_density
     uint32_t *walk_cost;       // [n] OG_COUNT only: interactions evaluated per target of the last walk, caller's order
     unsigned long long *d_counters;  // [OGC_N]
     // walk scratch (spill stacks), allocated lazily

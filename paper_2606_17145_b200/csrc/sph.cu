@@ -35,6 +35,7 @@ struct SphArgs {
     const uint2 *info;
     const uint32_t *node_first, *node_count, *first_child;
     const uint8_t *nchild;
+    const uint32_t *seed5;       // level-5 cell -> covering node (og_internal.cuh)
     const float4 *spos;
     const uint32_t *inv_perm, *perm;
     const uint32_t *active_idx;  // NULL: target k = sorted slot k, written at perm[k]
@@ -108,7 +109,36 @@ __device__ int sph_scan(const SphArgs &a, SphSmem &s, float px, float py, float 
     uint32_t *q = STORE ? s.q : reinterpret_cast<uint32_t *>(&s);
     const int qcap = STORE ? SPH_QCAP : (int)(sizeof(SphSmem) / sizeof(uint32_t));
     int qn = 1, cnt = 0;
-    if (lane == 0) q[0] = 0u;
+    {
+        // Entry points: the walk starts from the nodes that cover the level-5 cells the sphere's bounding box touches (at
+        // most 3 x 3 x 3 of them when the sphere is smaller than a cell; found in the tree's cell table, each node once),
+        // not from the root: the five upper levels of every walk are the same few nodes.
+        const float e = H * (1.0f + 1.0e-5f) + 2.0e-6f * a.L;
+        const float sc5 = 32.0f * a.invL;
+        const int x0 = (int)floorf((px - e) * sc5), x1 = (int)floorf((px + e) * sc5);
+        const int y0 = (int)floorf((py - e) * sc5), y1 = (int)floorf((py + e) * sc5);
+        const int z0 = (int)floorf((pz - e) * sc5), z1 = (int)floorf((pz + e) * sc5);
+        const int nx = x1 - x0 + 1, ny = y1 - y0 + 1, nz = z1 - z0 + 1;
+        if (nx <= 3 && ny <= 3 && nz <= 3) {
+            uint32_t node = 0xffffffffu;
+            if ((int)lane < nx * ny * nz) {
+                const int ix = (x0 + (int)lane % nx) & 31, iy = (y0 + ((int)lane / nx) % ny) & 31, iz = (z0 + (int)lane / (nx * ny)) & 31;
+                uint32_t m = 0u;
+#pragma unroll
+                for (int b = 0; b < 5; ++b)
+                    m |= (((uint32_t)ix >> b) & 1u) << (3 * b + 2) | (((uint32_t)iy >> b) & 1u) << (3 * b + 1) | (((uint32_t)iz >> b) & 1u) << (3 * b);
+                node = __ldg(a.seed5 + m);
+            }
+            const bool have = node != 0xffffffffu;
+            const uint32_t peers = __match_any_sync(0xffffffffu, node);
+            const bool first = have && (peers & lt) == 0u;            // a leaf above level 5 covers several cells: once
+            const uint32_t fb = __ballot_sync(0xffffffffu, first);
+            if (first) q[__popc(fb & lt)] = node;
+            qn = __popc(fb);
+        } else if (lane == 0) {
+            q[0] = 0u;
+        }
+    }
     __syncwarp();
     while (qn > 0) {
         const int take = min(qn, 32);
@@ -398,6 +428,7 @@ cudaError_t ogk_sph_density(const og_tree *t, const uint32_t *active_idx, uint64
     a.lo = t->node_lo; a.hi = t->node_hi; a.info = t->node_info;
     a.node_first = t->node_first; a.node_count = t->node_count; a.first_child = t->node_first_child;
     a.nchild = t->node_nchild;
+    a.seed5 = t->seed5;
     a.spos = t->spos; a.inv_perm = t->inv_perm; a.perm = t->perm;
     a.active_idx = active_idx; a.h_guess = h_guess;
     a.h_out = h_out; a.rho_out = rho_out; a.nn_out = nn_out;
