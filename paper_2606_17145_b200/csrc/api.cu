@@ -27,7 +27,7 @@ inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 struct Layout {
     size_t keysA, keysB, idxA, idxB, sort_scratch, spos, sh, inv_perm;
     size_t level, first, count, first_child, nchild, com, cell, lo, hi, info, rec;
-    size_t oct_scratch, level_start, status, counters, small_end, spill, cost, seed5, total;
+    size_t oct_scratch, level_start, status, counters, small_end, spill, cost, cover, total;
 };
 
 Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count, uint32_t spill_entries, bool count)
@@ -52,7 +52,7 @@ Layout make_layout(uint64_t n, uint32_t max_nodes, int sm_count, uint32_t spill_
     L.small_end = o;
     L.spill = take(ogk_walk_spill_bytes(sm_count, spill_entries));
     L.cost = take(count ? n * 4 : 0);
-    L.seed5 = take(32768 * 4);
+    L.cover = take(37449 * 4);
     L.total = o;
     return L;
 }
@@ -244,7 +244,7 @@ static og_tree *tree_build_impl(const float *pos, const float *mass, const float
     t->d_level_start = (uint32_t *)(b + L.level_start); t->d_status = (uint32_t *)(b + L.status);
     t->d_counters = (unsigned long long *)(b + L.counters);
     t->walk_cost = (params->flags & OG_COUNT) ? (uint32_t *)(b + L.cost) : nullptr;
-    t->seed5 = (uint32_t *)(b + L.seed5);
+    t->cover = (uint32_t *)(b + L.cover);
     t->walk_spill = b + L.spill; t->walk_spill_bytes = ogk_walk_spill_bytes(sms, t->walk_spill_cap);
 
 #define OG_BUILD_TRY(expr)                                                    \

@@ -349,19 +349,25 @@ k_upward(UpArgs a)
     }
 }
 
-// seed5[m] = the node that covers the level-5 cell with Morton index m: the node at level 5, or the leaf above it
-// (empty cells keep 0xffffffff).  One thread per node of the levels 0..5.
+// cover[off(l) + m] (l = 0..5, off(l) = (8^l - 1) / 7, m = Morton index of the cell at level l) = the node that covers
+// that cell: the node of level l, or the leaf above it; 0xffffffff for a cell without particles.  One thread per node of
+// the levels 0..5.  The walks use it to enter the tree at the level-5 cells around their targets (walk.cu, sph.cu).
 __global__ void __launch_bounds__(256)
-k_seed5(const uint64_t *__restrict__ keys, const uint8_t *__restrict__ level, const uint32_t *__restrict__ first,
-        const uint8_t *__restrict__ nchild, const uint32_t *__restrict__ level_start, uint32_t *__restrict__ seed5)
+k_cover(const uint64_t *__restrict__ keys, const uint8_t *__restrict__ level, const uint32_t *__restrict__ first,
+        const uint8_t *__restrict__ nchild, const uint32_t *__restrict__ level_start, uint32_t *__restrict__ cover)
 {
     const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= level_start[6]) return;
     const uint32_t lv = level[j];
-    if (lv < 5u && nchild[j] != 0u) return;          // covered by its descendants
-    const uint32_t shift = 3u * (5u - lv);
-    const uint32_t m0 = ((uint32_t)(keys[first[j]] >> 48) >> shift) << shift;
-    for (uint32_t m = m0; m < m0 + (1u << shift); ++m) seed5[m] = j;
+    const uint32_t m5 = (uint32_t)(keys[first[j]] >> 48);
+    const uint32_t off[6] = {0u, 1u, 9u, 73u, 585u, 4681u};
+    cover[off[lv] + (m5 >> (3u * (5u - lv)))] = j;
+    if (nchild[j] != 0u) return;
+    for (uint32_t l = lv + 1u; l <= 5u; ++l) {      // a leaf covers every cell below it
+        const uint32_t sh = 3u * (l - lv);
+        const uint32_t m0 = (m5 >> (3u * (5u - lv))) << sh;
+        for (uint32_t m = m0; m < m0 + (1u << sh); ++m) cover[off[l] + m] = j;
+    }
 }
 
 int coop_grid(const void *kernel, int threads, int sm_count)
@@ -405,8 +411,8 @@ cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st)
                                     dim3(coop_grid((const void *)k_upward, OCT_THREADS, t->sm_count)),
                                     dim3(OCT_THREADS), args2, 0, st);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(t->seed5, 0xff, 32768 * sizeof(uint32_t), st);
+    e = cudaMemsetAsync(t->cover, 0xff, 37449 * sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
-    k_seed5<<<(37449 + 255) / 256, 256, 0, st>>>(t->keys, t->node_level, t->node_first, t->node_nchild, t->d_level_start, t->seed5);
+    k_cover<<<(37449 + 255) / 256, 256, 0, st>>>(t->keys, t->node_level, t->node_first, t->node_nchild, t->d_level_start, t->cover);
     return cudaGetLastError();
 }

@@ -7,6 +7,7 @@
 #include "og.h"
 
 #define OG_MAX_LEVEL 21
+#define OG_COVER_L5 4681u     // offset of the level-5 cells in og_tree::cover
 
 // Latched device-side status bits (og_tree::d_status[0]).
 #define OG_DEV_NODE_OVERFLOW 1u
@@ -70,8 +71,8 @@ struct og_tree {
     // small device state
     uint32_t *d_level_start;   // [24]: start index per level, [22] = n_nodes, [23] = max level
     uint32_t *d_status;        // [16]: [0] latched status bits, [1] walk work counter, [2] sparse-active-list flag, [3] SPH ticket
-    uint32_t *seed5;           // [32768] level-5 cell (Morton index) -> the node that covers it (at level 5, or the leaf above;
-                               // 0xffffffff: empty cell); entry points of the neighbour walk of og_sph_density
+    uint32_t *cover;           // [37449] cell (level 0..5, Morton index; level l starts at (8^l - 1) / 7) -> the node that covers it
+                               // (of that level, or the leaf above; 0xffffffff: empty cell): entry points of the walks
     uint32_t *walk_cost;       // [n] OG_COUNT only: interactions evaluated per target of the last walk, caller's order
     unsigned long long *d_counters;  // [OGC_N]
     // walk scratch (spill stacks), allocated lazily

@@ -428,7 +428,7 @@ cudaError_t ogk_sph_density(const og_tree *t, const uint32_t *active_idx, uint64
     a.lo = t->node_lo; a.hi = t->node_hi; a.info = t->node_info;
     a.node_first = t->node_first; a.node_count = t->node_count; a.first_child = t->node_first_child;
     a.nchild = t->node_nchild;
-    a.seed5 = t->seed5;
+    a.seed5 = t->cover + OG_COVER_L5;
     a.spos = t->spos; a.inv_perm = t->inv_perm; a.perm = t->perm;
     a.active_idx = active_idx; a.h_guess = h_guess;
     a.h_out = h_out; a.rho_out = rho_out; a.nn_out = nn_out;
