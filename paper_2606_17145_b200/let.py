@@ -121,19 +121,38 @@ def decompose(B, parts: dict, ex, box: float):
         g = p.gid.to(torch.int64)
         row = torch.cat([p.pos, p.mass[:, None], p.eps[:, None], act[:, None], ao[:, None],
                          (g >> 24).to(torch.float32)[:, None], (g & 0xFFFFFF).to(torch.float32)[:, None]], 1)
-        send[r] = [row[own == q].contiguous() for q in range(ex.R)]
+        send[r] = _split_by_owner(B, row, own, ex.R)
     recv = ex.alltoall(send)
     out = {}
     for r in ex.ranks:
         row = torch.cat(recv[r], 0)
         gid = (row[:, 7].to(torch.int64) << 24) | row[:, 8].to(torch.int64)
-        row = row[torch.argsort(gid)]
-        gid = torch.sort(gid).values
+        gid, order = _sort_by_key(B, gid)
+        row = row[order]
         act = torch.nonzero(row[:, 5] > 0).flatten().to(torch.int32)
         has_aold = any(parts[q].a_old is not None for q in ex.ranks)
         out[r] = Domain(row[:, 0:3].contiguous(), row[:, 3].contiguous(), row[:, 4].contiguous(), gid, act,
                         row[:, 6][act.long()].contiguous() if has_aold else None)
     return out, S
+
+
+def _sort_by_key(B, key: torch.Tensor):
+    """Ascending order of int64 keys >= 0 -> (sorted keys, order as int64 indices): the library's radix sort on the device
+    (row a2), torch.sort for the CPU tensors of the plumbing tests."""
+    n = int(key.shape[0])
+    if n == 0 or not key.is_cuda or not hasattr(B, "og_radix_sort_pairs"):
+        ks, order = torch.sort(key, stable=True)
+        return ks, order
+    bits = max(1, int(key.max().item()).bit_length())
+    ks, vs = B.og_radix_sort_pairs(key.clone(), torch.arange(n, dtype=torch.int32, device=key.device), 0, bits)
+    return ks, vs.long()
+
+
+def _split_by_owner(B, row: torch.Tensor, own: torch.Tensor, n_domains: int):
+    """rows grouped by owner (one stable sort on the owner + one gather) -> list over the destinations."""
+    _, order = _sort_by_key(B, own.to(torch.int64))
+    cnt = torch.bincount(own.long(), minlength=n_domains).tolist()
+    return [x.contiguous() for x in torch.split(row[order], cnt, 0)]
 
 
 def top_boxes(B, tree, level: int = 2) -> torch.Tensor:
