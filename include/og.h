@@ -286,7 +286,8 @@ int og_ts_kick(float *vel, uint8_t *bin, float *a_old, const uint32_t *active_id
  *              starts at 1.05 x this; any positive value reaches the same root), or NULL -> derived from the tree (the
  *              radius that holds 1.5 n_des at the mean density of the deepest ancestor cell with n_des particles)
  *   h_out      DEVICE f32 [n_active]; rho_out, nn_out (N at the returned h): DEVICE f32 [n_active] or NULL
- * Enqueues on `stream` (ordered after the tree's build).  Neighbour candidates are kept in a per-warp list of 512
+ * Enqueues on `stream` (ordered after the tree's build and the previous call on the tree; the first call on a tree also
+ * writes the tree's table of level-5 cells, where the neighbour walks start).  Neighbour candidates are kept in a per-warp list of 512
  * entries; a target whose root sphere holds more (a void particle whose kernel rim grazes a dense clump) is solved
  * by re-walking the tree for every trial h instead (same result, slower).  A target with more than 3 n_des / 32
  * coincident particles (N(h) > n_des for every h: no root), or whose pending nodes exceed even the fallback's stack,

@@ -345,10 +345,16 @@ extern "C" int og_sph_density(const og_tree *t, const uint32_t *active_idx, uint
     }
     cudaStream_t st = (cudaStream_t)stream;
     if (st != t->build_stream) OG_CUDA_TRY(cudaStreamWaitEvent(st, t->ev_built, 0), return OG_ERR_CUDA);
+    // the cell table of the tree is written by the first call (calls on one tree from several host threads at once are not
+    // supported, og.h; a later call on another stream is ordered after this one by the tree's event below)
+    if (t->walked) OG_CUDA_TRY(cudaStreamWaitEvent(st, t->ev_walked, 0), return OG_ERR_CUDA);
+    if (!t->cover_built) {
+        OG_CUDA_TRY(ogk_cover(t, st), return OG_ERR_CUDA);
+        t->cover_built = true;
+    }
     OG_CUDA_TRY(ogk_sph_density(t, active_idx, n_active, n_des, tol_n, h_guess, h_out, rho_out, nn_out, st),
                 return OG_ERR_CUDA);
     // og_tree_free and og_tree_status wait for this call like for a walk
-    if (t->walked) OG_CUDA_TRY(cudaStreamWaitEvent(st, t->ev_walked, 0), return OG_ERR_CUDA);
     OG_CUDA_TRY(cudaEventRecord(t->ev_walked, st), return OG_ERR_CUDA);
     t->walked = true;
     return OG_OK;

@@ -351,7 +351,7 @@ k_upward(UpArgs a)
 
 // cover[off(l) + m] (l = 0..5, off(l) = (8^l - 1) / 7, m = Morton index of the cell at level l) = the node that covers
 // that cell: the node of level l, or the leaf above it; 0xffffffff for a cell without particles.  One thread per node of
-// the levels 0..5.  The walks use it to enter the tree at the level-5 cells around their targets (walk.cu, sph.cu).
+// the levels 0..5.  The neighbour walk of og_sph_density enters the tree at the level-5 cells around its target (sph.cu).
 __global__ void __launch_bounds__(256)
 k_cover(const uint64_t *__restrict__ keys, const uint8_t *__restrict__ level, const uint32_t *__restrict__ first,
         const uint8_t *__restrict__ nchild, const uint32_t *__restrict__ level_start, uint32_t *__restrict__ cover)
@@ -410,8 +410,13 @@ cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st)
     e = cudaLaunchCooperativeKernel((const void *)k_upward,
                                     dim3(coop_grid((const void *)k_upward, OCT_THREADS, t->sm_count)),
                                     dim3(OCT_THREADS), args2, 0, st);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(t->cover, 0xff, 37449 * sizeof(uint32_t), st);
+    return e;
+}
+
+// The cell table is written on first use (og_sph_density): a gravity-only step does not pay for it.
+cudaError_t ogk_cover(const og_tree *t, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(t->cover, 0xff, 37449 * sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
     k_cover<<<(37449 + 255) / 256, 256, 0, st>>>(t->keys, t->node_level, t->node_first, t->node_nchild, t->d_level_start, t->cover);
     return cudaGetLastError();

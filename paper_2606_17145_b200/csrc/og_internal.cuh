@@ -85,6 +85,7 @@ struct og_tree {
     cudaEvent_t ev_built;
     cudaEvent_t ev_walked;
     mutable bool walked;
+    mutable bool cover_built;  // the cell table has been written (by the first og_sph_density on this tree)
     mutable int64_t n_nodes_host;   // -1 until read back
     mutable uint32_t max_level_host;
 };
@@ -117,6 +118,7 @@ cudaError_t ogk_gather(const float *pos, const float *mass, const float *soft,
 // a4 + a5
 size_t ogk_octree_scratch_bytes(uint32_t max_nodes);
 cudaError_t ogk_octree_upward(og_tree *t, void *scratch, cudaStream_t st);
+cudaError_t ogk_cover(const og_tree *t, cudaStream_t st);
 // a6 + a7
 cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out,
                      uint64_t n_active, const float *a_old, float *acc_out, float *pot_out,
