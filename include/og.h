@@ -200,6 +200,30 @@ int og_radix_sort_pairs(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint
                         size_t scratch_bytes, int *result_in_alt, og_stream stream);
 
 /*
+ * Row a2 for callers that cannot allocate device memory: the same sort, same result bit for bit, but without a
+ * scratch argument and without a single allocation inside the library (no cudaMalloc / cudaFree / cudaMallocAsync,
+ * no library routine that allocates).  Who needs this: a simulation code that claims the whole device for its own
+ * arena at start-up and has nothing left to allocate from; a step that runs where an allocation would stall or
+ * deadlock (another thread holds the allocator, or the allocation would synchronise the device in the middle of
+ * overlapped work); a component that is only lent buffers and owns no allocator.  Such a caller can still pass the four
+ * ping-pong buffers -- those are its inputs and outputs -- but not a scratch buffer sized per call.
+ *   The scratch (digit histograms, tile tickets and look-back words of the one-sweep passes) lives in a fixed array
+ * compiled into the library: every GPU on which libogtree.so is loaded carries it (about 4 MiB) until the process
+ * exits, whether or not this call is ever used.  That fixes the limit: n <= OG_SORT_NOALLOC_MAX_N.  A larger n is
+ * refused with OG_ERR_INVALID_ARG and a message naming the limit; nothing is enqueued.  Use og_radix_sort_pairs then.
+ *   keys / vals / keys_alt / vals_alt, begin_bit, end_bit, result_in_alt, stream: exactly as og_radix_sort_pairs.
+ *   First call on a device: the library looks up the array's device address (cudaGetSymbolAddress, with the caller's
+ * current device) and remembers it per device.  The runtime may load the library's device code at that moment, so
+ * make the first call on each device during set-up, before any stream capture begins.
+ *   Sharing: all calls on one device use the same array.  Each call zeroes what it needs on `stream` before its
+ * kernels run, so a call never depends on what an earlier one left there.  Calls that can be in flight on the GPU at
+ * the same time (two streams, two host threads) race on the array: order them (one stream, or events).
+ */
+#define OG_SORT_NOALLOC_MAX_N 1048576u   /* 2^20 pairs */
+int og_radix_sort_pairs_noalloc(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint32_t *vals_alt, uint64_t n,
+                                int begin_bit, int end_bit, int *result_in_alt, og_stream stream);
+
+/*
  * End-to-end convenience with HOST buffers (bench.py's `e2e` leg): copies pos/mass/soft
  * (and active_idx, a_old if given) to the device, runs og_tree_build + og_shortrange_accel,
  * copies acc/pot back, frees everything, and synchronises `stream` before returning.

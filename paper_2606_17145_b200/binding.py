@@ -101,6 +101,8 @@ def _load():
     lib.og_radix_sort_pairs.restype = C.c_int
     lib.og_radix_sort_pairs.argtypes = [vp, vp, vp, vp, u64, C.c_int, C.c_int, vp, C.c_size_t,
                                         C.POINTER(C.c_int), vp]
+    lib.og_radix_sort_pairs_noalloc.restype = C.c_int
+    lib.og_radix_sort_pairs_noalloc.argtypes = [vp, vp, vp, vp, u64, C.c_int, C.c_int, C.POINTER(C.c_int), vp]
     lib.og_shortrange_accel_host.restype = C.c_int
     lib.og_shortrange_accel_host.argtypes = [vp, vp, vp, u64, C.c_float, C.POINTER(og_params), vp, u64, vp, vp,
                                              vp, vp]
@@ -141,7 +143,7 @@ _lib = _load()
 
 EXPORTS = ("og_tree_workspace_bytes", "og_tree_build", "og_shortrange_accel", "og_tree_get", "og_tree_status",
            "og_tree_stats", "og_tree_free", "og_last_error", "og_morton_keys", "og_radix_sort_scratch_bytes",
-           "og_radix_sort_pairs", "og_shortrange_accel_host", "og_trim", "og_pm_create", "og_pm_longrange",
+           "og_radix_sort_pairs", "og_radix_sort_pairs_noalloc", "og_shortrange_accel_host", "og_trim", "og_pm_create", "og_pm_longrange",
            "og_pm_free", "og_ts_scratch_bytes", "og_ts_drift", "og_ts_next_tick", "og_ts_active_list", "og_ts_kick",
            "og_sph_density", "og_shortrange_accel_ext", "og_domain_cell_hist", "og_domain_owner", "og_let_export_list",
            "og_let_accumulate")
@@ -300,6 +302,27 @@ def og_radix_sort_pairs(keys: torch.Tensor, vals: torch.Tensor, begin_bit: int =
                                     scratch.numel(), C.byref(in_alt), _stream(stream)))
     torch.cuda.current_stream().synchronize()  # scratch must outlive the sort
     return (k2, v2) if in_alt.value else (keys, vals)
+
+
+OG_SORT_NOALLOC_MAX_N = 1 << 20
+
+
+def og_radix_sort_pairs_noalloc(keys: torch.Tensor, vals: torch.Tensor, keys_alt: torch.Tensor, vals_alt: torch.Tensor,
+                                begin_bit: int = 0, end_bit: int = 64, stream=None):
+    """Row a2 without any allocation (og.h: og_radix_sort_pairs_noalloc): for callers that own all their device memory
+    up front and cannot allocate a per-call scratch.  The caller passes all four ping-pong buffers (keys int64 = u64 bit
+    pattern, vals int32, n <= OG_SORT_NOALLOC_MAX_N each); the scratch is the library's built-in array, shared by every
+    call on the device, so calls must not overlap on the GPU.  Nothing is allocated here either: the return value is
+    the pair of the caller's own tensors that holds the sorted data, (keys_alt, vals_alt) or (keys, vals).  Make the
+    first call on a device outside a stream capture (the library resolves the array's address then)."""
+    n = int(keys.shape[0])
+    if int(vals.shape[0]) != n or int(keys_alt.shape[0]) < n or int(vals_alt.shape[0]) < n:
+        raise ValueError("og_radix_sort_pairs_noalloc: vals / keys_alt / vals_alt must hold n elements")
+    in_alt = C.c_int(0)
+    _check(_lib.og_radix_sort_pairs_noalloc(_dev(keys, torch.int64, "keys"), _dev(vals, torch.int32, "vals"),
+                                            _dev(keys_alt, torch.int64, "keys_alt"), _dev(vals_alt, torch.int32, "vals_alt"),
+                                            n, begin_bit, end_bit, C.byref(in_alt), _stream(stream)))
+    return (keys_alt, vals_alt) if in_alt.value else (keys, vals)
 
 
 def og_shortrange_accel_host(pos, mass, soft, box: float, params: og_params, active_idx=None, a_old=None,

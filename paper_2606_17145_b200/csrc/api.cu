@@ -584,6 +584,28 @@ extern "C" int og_radix_sort_pairs(uint64_t *keys, uint32_t *vals, uint64_t *key
     return OG_OK;
 }
 
+// The variant of og_radix_sort_pairs whose scratch is a fixed array inside the library (radix_sort.cu): argument checks
+// here, nothing allocated anywhere on the path.
+extern "C" int og_radix_sort_pairs_noalloc(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint32_t *vals_alt,
+                                           uint64_t n, int begin_bit, int end_bit, int *result_in_alt, og_stream stream)
+{
+    g_err[0] = 0;
+    if (!keys || !vals || !keys_alt || !vals_alt || n == 0 || begin_bit < 0 || end_bit > 64 || begin_bit >= end_bit) {
+        og_set_error("og_radix_sort_pairs_noalloc: bad argument");
+        return OG_ERR_INVALID_ARG;
+    }
+    if (n > (uint64_t)ogk_sort_noalloc_max_n()) {
+        og_set_error("og_radix_sort_pairs_noalloc: n = %llu exceeds OG_SORT_NOALLOC_MAX_N = %llu, the capacity of the "
+                     "library's built-in scratch array (use og_radix_sort_pairs with caller-supplied scratch)",
+                     (unsigned long long)n, (unsigned long long)ogk_sort_noalloc_max_n());
+        return OG_ERR_INVALID_ARG;
+    }
+    OG_CUDA_TRY(ogk_radix_sort_noalloc(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, result_in_alt,
+                                       (cudaStream_t)stream),
+                return OG_ERR_CUDA);
+    return OG_OK;
+}
+
 extern "C" int og_shortrange_accel_host(const float *pos, const float *mass, const float *soft, uint64_t n,
                                         float box, const og_params *params, const uint32_t *active_idx,
                                         uint64_t n_active, const float *a_old, float *acc_out, float *pot_out,

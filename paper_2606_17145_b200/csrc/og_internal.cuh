@@ -111,6 +111,10 @@ size_t ogk_sort_scratch_bytes(uint64_t n);
 cudaError_t ogk_radix_sort(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint32_t *vals_alt,
                            uint64_t n, int begin_bit, int end_bit, void *scratch, int *in_alt,
                            cudaStream_t st);
+// a2 with the scratch in a fixed array of the library image (og_radix_sort_pairs_noalloc)
+size_t ogk_sort_noalloc_max_n(void);
+cudaError_t ogk_radix_sort_noalloc(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint32_t *vals_alt, uint64_t n,
+                                   int begin_bit, int end_bit, int *in_alt, cudaStream_t st);
 // a3
 cudaError_t ogk_gather(const float *pos, const float *mass, const float *soft,
                        const uint32_t *perm, uint64_t n, float4 *spos, float *sh,

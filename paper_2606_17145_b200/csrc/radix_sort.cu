@@ -467,3 +467,63 @@ cudaError_t ogk_radix_sort(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, u
     }
     return cudaGetLastError();
 }
+
+// ---- og_radix_sort_pairs_noalloc: the same sort with its scratch inside the library --------------------------------
+// For callers that must not allocate device memory at the moment they need a sort: a host code whose device memory
+// was handed out in full at start-up to its own arena, a step that runs while another thread holds the allocator,
+// a plug-in that is only lent buffers.  They cannot supply og_radix_sort_pairs' scratch from a fresh cudaMalloc, so
+// the scratch of this variant (digit histograms, tile tickets, look-back status words of the one-sweep passes) is a
+// fixed array in the library image: OG_SORT_NOALLOC_MAX_N pairs at most, about 4 MiB, resident on every GPU that
+// loads libogtree.so for as long as the process lives.
+//
+// The array is one object shared by every call on a device.  ogk_radix_sort zeroes the part a call uses (cudaMemsetAsync
+// on the caller's stream) before its kernels run, so what the previous call left behind never matters; two calls
+// that are in flight on the GPU at the same time (different streams, or different host threads) would overwrite
+// each other's status words and must be ordered by the caller.
+//
+// g_sort_noalloc_scratch below is a DEVICE object.  In host code its name is only the host-side handle of the
+// symbol, never an address a kernel may dereference; the device address is asked for once per device with
+// cudaGetSymbolAddress (with that device current) and kept in g_noalloc_ptr[].  That first call per device may make
+// the runtime load this module, which is why og.h asks for it to happen outside a stream capture.
+#include <mutex>
+
+namespace {
+constexpr uint64_t NOALLOC_MAX_N = OG_SORT_NOALLOC_MAX_N;
+constexpr size_t NOALLOC_TILES = (NOALLOC_MAX_N + SORT_TILE - 1) / SORT_TILE;
+constexpr size_t NOALLOC_BYTES =
+    ((size_t)SORT_MAX_PASSES * 256 + 64 + (size_t)SORT_MAX_PASSES * NOALLOC_TILES * 256) * sizeof(uint32_t) + 256;
+constexpr int NOALLOC_MAX_DEVICES = 64;
+void *g_noalloc_ptr[NOALLOC_MAX_DEVICES];   // device address of the array on device d, 0 until asked for
+std::mutex g_noalloc_mu;
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_sort_noalloc_scratch[NOALLOC_BYTES];
+
+size_t ogk_sort_noalloc_max_n(void) { return (size_t)NOALLOC_MAX_N; }
+
+// Resolves the array's address on the current device (first call per device only), then runs the unchanged sort on
+// it.  Calls nothing that allocates: cudaGetDevice, cudaGetSymbolAddress, cudaFuncSetAttribute, cudaMemsetAsync and
+// kernel launches.  n <= OG_SORT_NOALLOC_MAX_N is the caller's (api.cu's) check; it is repeated here because an
+// overrun of a file-scope array would corrupt whatever the linker placed behind it.
+cudaError_t ogk_radix_sort_noalloc(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, uint32_t *vals_alt, uint64_t n,
+                                   int begin_bit, int end_bit, int *in_alt, cudaStream_t st)
+{
+    if (n > NOALLOC_MAX_N || ogk_sort_scratch_bytes(n) > NOALLOC_BYTES) return cudaErrorInvalidValue;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    void *scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mu);
+        if (!g_noalloc_ptr[dev]) {
+            void *p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_sort_noalloc_scratch);
+            if (e != cudaSuccess) return e;
+            if (!p) return cudaErrorInvalidSymbol;
+            g_noalloc_ptr[dev] = p;
+        }
+        scratch = g_noalloc_ptr[dev];
+    }
+    return ogk_radix_sort(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, scratch, in_alt, st);
+}
