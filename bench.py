@@ -309,7 +309,12 @@ def run_ours(args):
         torch.cuda.synchronize()
         cost = B.og_tree_get(tc, B.OG_F_WALK_COST).cpu().numpy().view(np.uint32)[:na]
         inv_perm = B.og_tree_get(tc, B.OG_F_INV_PERM).cpu().numpy().view(np.uint32)
+        # a rank's share is walked with the grouping the full list got (og.h: the bits of a sub-list equal the full
+        # call's only under the same grouping, and the automatic choice looks at each list's own Morton span)
+        tpw = B.og_tree_stats(tc)["walk_targets_per_warp"]
         B.og_tree_free(tc)
+        if w.active_idx is not None:
+            prm.flags |= B.OG_WALK_G8 if tpw == 8 else B.OG_WALK_G32
         slots = inv_perm if w.active_idx is None else inv_perm[w.active_idx]
         order = S.sorted_active_order(slots)
         bounds = S.partition_by_cost(cost[order], world)
@@ -365,6 +370,9 @@ def run_ours(args):
         # every rank's share equals the single-call result bit for bit (whole warps of the same sorted order)
         ok = bool(torch.equal(acc, full_acc[my_pos_d]) and torch.equal(pot, full_pot[my_pos_d]))
         shard["bitwise_equal_to_single_call"] = bool(all_max(0.0 if ok else 1.0, dev) == 0.0)
+        shard["targets_per_warp"] = int(tpw)
+        if not shard["bitwise_equal_to_single_call"]:
+            raise SystemExit("bench.py --scaling strong: a rank's share differs from the single-call result")
         h_act = torch.from_numpy(my_idx.view(np.int32)).pin_memory()
         del full_acc, full_pot
     # e2e through the HOST-buffer entry point (pinned inputs, H2D + build + walk + D2H inside)

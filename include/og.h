@@ -59,6 +59,9 @@ typedef enum {
 #define OG_PERIODIC 1u      /* required in this build (nearest-image distances, R13)      */
 #define OG_VALIDATE_POS 2u  /* device-side check 0 <= x < box during key generation       */
 #define OG_COUNT 4u         /* walk also accumulates interaction counters (og_stats)      */
+#define OG_WALK_G32 8u      /* og_shortrange_accel with an active list: always 32 targets per warp ...       */
+#define OG_WALK_G8 16u      /* ... always 8 targets per warp (neither bit: chosen per call from the list, see  */
+                            /* og_shortrange_accel; both bits: invalid)                                         */
 
 typedef struct {
     uint32_t struct_size;   /* = sizeof(og_params); ABI guard                              */
@@ -84,7 +87,7 @@ typedef struct {
     uint64_t n;             /* particles                                                   */
     uint64_t n_nodes;       /* nodes of the canonical octree                               */
     uint32_t max_level;     /* deepest level holding a node (root = 0)                     */
-    uint32_t reserved;
+    uint32_t walk_targets_per_warp;  /* grouping the last og_shortrange_accel on this tree used: 32 or 8 (0: no walk yet) */
     /* sums over the targets of the last og_shortrange_accel with OG_COUNT (else 0):       */
     uint64_t V_full;        /* visits that passed the cull                                 */
     uint64_t V_cull;        /* visits removed by the cutoff-box test                       */
@@ -157,10 +160,15 @@ og_tree *og_tree_build(const float *pos, const float *mass, const float *soft, u
  * Returns OG_OK or a negative og_status; conditions detected on the device (bad index, traversal stack
  * capacity) are latched and reported by og_tree_status().  n_active == 0 is a no-op.  Implementation note:
  * the targets are taken in Morton order, 32 per warp; an active list that fills fewer than 1 / 16 of the Morton
- * range it covers is walked with 8 targets per warp (4 lanes per target), decided on the device.  Results do not
- * depend on the launch order (bit-reproducible run to run), and a call on a sub-list that covers whole warps of
- * the full list's order (a multiple of 32 consecutive targets of the sorted active list) returns the same bits as
- * the full call does for those targets.
+ * range it covers is walked with 8 targets per warp (4 lanes per target), decided on the device from THAT list's
+ * first and last target (OG_WALK_G32 / OG_WALK_G8 in og_params.flags fix the grouping instead; og_stats.
+ * walk_targets_per_warp tells which one the last call used).  Results do not depend on the launch order
+ * (bit-reproducible run to run), and a call on a sub-list that covers whole warps of the full list's order (a
+ * multiple of 32 consecutive targets of the sorted active list) returns the same bits as the full call does for those
+ * targets PROVIDED both calls use the same grouping: the partial sums of a target are added in an order that depends
+ * on it.  The automatic choice does not guarantee that (a list made of two distant clumps counts as sparse, each clump
+ * alone as dense), so a caller who splits a list over several calls or ranks builds the sub-list trees with the flag
+ * that matches the full call's og_stats.walk_targets_per_warp (bench.py --scaling strong does).
  */
 int og_shortrange_accel(const og_tree *tree, const uint32_t *active_idx, uint64_t n_active,
                         const float *a_old, float *acc_out, float *pot_out, og_stream stream);

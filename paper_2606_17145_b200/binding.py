@@ -28,6 +28,8 @@ OG_ERR_NGB_OVERFLOW = -7
 OG_PERIODIC = 1
 OG_VALIDATE_POS = 2
 OG_COUNT = 4
+OG_WALK_G32 = 8
+OG_WALK_G8 = 16
 # og_field
 (OG_F_KEYS_SORTED, OG_F_PERM, OG_F_INV_PERM, OG_F_SPOS, OG_F_SH, OG_F_NODE_LEVEL, OG_F_NODE_FIRST,
  OG_F_NODE_COUNT, OG_F_NODE_FIRST_CHILD, OG_F_NODE_NCHILD, OG_F_NODE_COM, OG_F_NODE_CELL, OG_F_NODE_LO,
@@ -55,7 +57,7 @@ class og_params(C.Structure):
 
 
 class og_stats(C.Structure):
-    _fields_ = [("n", C.c_uint64), ("n_nodes", C.c_uint64), ("max_level", C.c_uint32), ("reserved", C.c_uint32),
+    _fields_ = [("n", C.c_uint64), ("n_nodes", C.c_uint64), ("max_level", C.c_uint32), ("walk_targets_per_warp", C.c_uint32),
                 ("V_full", C.c_uint64), ("V_cull", C.c_uint64), ("A_in", C.c_uint64), ("P_in", C.c_uint64),
                 ("P_soft", C.c_uint64), ("P_out", C.c_uint64), ("fp64_rechecks", C.c_uint64),
                 ("cl_drop", C.c_uint64), ("cl_open", C.c_uint64), ("cl_accept", C.c_uint64),
@@ -63,7 +65,7 @@ class og_stats(C.Structure):
                 ("pt_wrap", C.c_uint64), ("batches", C.c_uint64), ("stack_spills", C.c_uint64)]
 
     def as_dict(self):
-        return {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}
+        return {k: int(getattr(self, k)) for k, _ in self._fields_ }
 
 
 def make_params(r_s, G=1.0, rcut_over_rs=4.5, alpha=0.005, theta=0.5, leaf_max=8, max_nodes=0, flags=OG_PERIODIC,

@@ -77,6 +77,10 @@ bool check_params(const og_params *p, uint64_t n, float box)
     if (n == 0 || n >= (1ull << 31)) { og_set_error("n = %llu out of range [1, 2^31)", (unsigned long long)n); return false; }
     if (!(box > 0.0f)) { og_set_error("box must be > 0"); return false; }
     if (!(p->flags & OG_PERIODIC)) { og_set_error("OG_PERIODIC is required in this build"); return false; }
+    if ((p->flags & OG_WALK_G32) && (p->flags & OG_WALK_G8)) {
+        og_set_error("OG_WALK_G32 and OG_WALK_G8 exclude each other");
+        return false;
+    }
     if (p->leaf_max == 0) { og_set_error("leaf_max must be >= 1"); return false; }
     if (!(p->r_s > 0.0f) || !(p->rcut_over_rs > 0.0f)) { og_set_error("r_s and rcut_over_rs must be > 0"); return false; }
     if (p->rcut_over_rs > 5.0f) {
@@ -295,6 +299,7 @@ extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx,
         OG_CUDA_TRY(ogk_walk(t, nullptr, t->perm, n_active, a_old, acc_out, pot_out, st), return OG_ERR_CUDA);
         OG_CUDA_TRY(cudaEventRecord(t->ev_walked, st), return OG_ERR_CUDA);
         t->walked = true;
+        t->walk_kind = 1;
         return OG_OK;
     }
     // active subset: order the targets by sorted slot so that a warp's 32 targets are neighbours
@@ -317,10 +322,14 @@ extern "C" int og_shortrange_accel(const og_tree *t, const uint32_t *active_idx,
 #define OG_ACC_TRY(expr) OG_CUDA_TRY(expr, { cudaFreeAsync(tmp, st); return OG_ERR_CUDA; })
     OG_ACC_TRY(ogk_active_slots(active_idx, t->inv_perm, t->n, n_active, k0, v0, t->d_status, st));
     OG_ACC_TRY(ogk_radix_sort(k0, v0, k1, v1, n_active, 0, bits, tmp + o_sc, &in_alt, st));
-    OG_ACC_TRY(ogk_unpack_slots(in_alt ? k1 : k0, n_active, slots, OG_SPARSE_DIV, t->d_status + 2, st));
+    // grouping (og.h): n_active * div < span of the list in sorted slots -> 8 targets per warp.  The flags fix it through
+    // the divisor: 0 makes the test true for every list, 2^32 - 1 false (n_active >= 1, span <= n < 2^31)
+    const uint32_t sparse_div = (t->prm.flags & OG_WALK_G8) ? 0u : (t->prm.flags & OG_WALK_G32) ? 0xffffffffu : OG_SPARSE_DIV;
+    OG_ACC_TRY(ogk_unpack_slots(in_alt ? k1 : k0, n_active, slots, sparse_div, t->d_status + 2, st));
     OG_ACC_TRY(ogk_walk(t, slots, in_alt ? v1 : v0, n_active, a_old, acc_out, pot_out, st));
     OG_ACC_TRY(cudaEventRecord(t->ev_walked, st));
     t->walked = true;
+    t->walk_kind = 2;
     OG_ACC_TRY(cudaFreeAsync(tmp, st));
 #undef OG_ACC_TRY
     return OG_OK;
@@ -396,6 +405,7 @@ extern "C" int og_shortrange_accel_ext(const og_tree *t, const float *tpos, cons
     OG_EXT_TRY(ogk_walk(t, nullptr, order, n_t, a_old, acc_out, pot_out, st, ext));
     OG_EXT_TRY(cudaEventRecord(t->ev_walked, st));
     t->walked = true;
+    t->walk_kind = 1;
     OG_EXT_TRY(cudaFreeAsync(tmp, st));
 #undef OG_EXT_TRY
     return OG_OK;
@@ -539,6 +549,13 @@ extern "C" int og_tree_stats(const og_tree *t, og_stats *out)
     out->cl_generic = c[OGC_CL_GENERIC]; out->pt_drop = c[OGC_PT_DROP]; out->pt_shift = c[OGC_PT_SHIFT];
     out->pt_wrap = c[OGC_PT_WRAP]; out->batches = c[OGC_BATCHES];
     out->stack_spills = c[OGC_SPILLS];
+    if (t->walk_kind == 2) {
+        uint32_t sparse = 0;
+        OG_CUDA_TRY(cudaMemcpy(&sparse, t->d_status + 2, sizeof(sparse), cudaMemcpyDeviceToHost), return OG_ERR_CUDA);
+        out->walk_targets_per_warp = sparse ? 8u : 32u;
+    } else {
+        out->walk_targets_per_warp = t->walk_kind == 1 ? 32u : 0u;
+    }
     return OG_OK;
 }
 

@@ -85,6 +85,8 @@ struct og_tree {
     cudaEvent_t ev_built;
     cudaEvent_t ev_walked;
     mutable bool walked;
+    mutable int walk_kind;     // last og_shortrange_accel[_ext]: 0 none yet, 1 identity list / external targets (32 per warp),
+                               // 2 explicit active list (d_status[2] holds the choice: 0 -> 32, 1 -> 8 targets per warp)
     mutable bool cover_built;  // the cell table has been written (by the first og_sph_density on this tree)
     mutable int64_t n_nodes_host;   // -1 until read back
     mutable uint32_t max_level_host;

@@ -3,7 +3,10 @@ tree exists every active target is independent, so each rank holds the whole tre
 inputs) and walks a contiguous MORTON range of the active targets, balanced by the work each target took in the
 previous pass (OG_F_WALK_COST).  No reduction: every target has one owner.  Range boundaries are multiples of 32
 positions of the sorted active order, so that every rank's warps hold exactly the targets they would hold in a
-single-GPU call and the concatenated results are bit-identical to it (og.h, og_shortrange_accel).
+single-GPU call and the concatenated results are bit-identical to it (og.h, og_shortrange_accel) -- provided every
+rank walks with the grouping the full list would get: the library picks 32 or 8 targets per warp from each list's own
+Morton span, so the ranks build their trees with OG_WALK_G32 / OG_WALK_G8 as og_stats.walk_targets_per_warp of a call
+on the full list says (bench.py --scaling strong).
 
 Pure NumPy index logic: no method arithmetic, no CUDA (the world-size-2 gloo test runs it on CPU)."""
 from __future__ import annotations

@@ -334,3 +334,60 @@ def test_sublist_of_whole_warps_returns_the_same_bits_and_cost_field(B):
     with pytest.raises(B.OgError):
         B.og_tree_get(tree, B.OG_F_WALK_COST)
     B.og_tree_free(tree)
+
+
+def test_sparse_full_list_and_its_sub_ranges_agree_under_the_same_grouping(B):
+    """og.h (og_shortrange_accel): the bits of a whole-warp sub-list equal the full call's PROVIDED both use the same
+    grouping.  A list of two dense clumps at the two ends of the Morton curve counts as sparse (8 targets per warp),
+    each clump alone as dense (32 per warp): the automatic choice differs, og_stats.walk_targets_per_warp says so, and
+    OG_WALK_G8 / OG_WALK_G32 on the sub-list's tree restore the full call's bits."""
+    import torch
+    w = W.make("nfw256", small=True)
+    pos, mass, eps = (torch.from_numpy(x).cuda() for x in (w.pos, w.mass, w.eps))
+
+    def build(extra=0):
+        return B.og_tree_build(pos, mass, eps, w.L, B.make_params(w.r_s, G=w.G, alpha=w.alpha, theta=w.theta,
+                                                                  flags=B.OG_PERIODIC | extra))
+    tree = build()
+    assert B.og_tree_stats(tree)["walk_targets_per_warp"] == 0            # no walk yet
+    a_id, p_id = B.og_shortrange_accel(tree, None, None)                  # identity list: 32 per warp
+    assert B.og_tree_stats(tree)["walk_targets_per_warp"] == 32
+    perm = B.og_tree_get(tree, B.OG_F_PERM).cpu().numpy().view(np.uint32)
+    n, m = w.n, 32 * 20
+    clump_a, clump_b = perm[:m].copy(), perm[n - m:].copy()               # sorted slots [0, m) and [n - m, n)
+    full = np.concatenate([clump_b, clump_a])                             # any order: the library sorts by slot
+    np.random.default_rng(5).shuffle(full)
+    assert full.size * 16 < n                                             # the rule of og.h: sparse
+    dev = lambda x: torch.from_numpy(np.ascontiguousarray(x).view(np.int32)).cuda()
+    a_full, p_full = B.og_shortrange_accel(tree, dev(full), None)
+    assert B.og_tree_stats(tree)["walk_targets_per_warp"] == 8
+    res = {int(i): (a_full[k].clone(), float(p_full[k])) for k, i in enumerate(full)}
+
+    def same_bits(a, p, idx, ref_a=None):
+        for k, i in enumerate(idx):
+            ra, rp = res[int(i)]
+            if not (torch.equal(a[k], ra) and float(p[k]) == rp):
+                return False
+        return True
+
+    # automatic choice on a clump alone: dense -- a different grouping than the full call's (bits are then not promised)
+    B.og_shortrange_accel(tree, dev(clump_a), None)
+    assert B.og_tree_stats(tree)["walk_targets_per_warp"] == 32
+    B.og_tree_free(tree)
+    # the full call's grouping fixed by the flag: the clumps and 32-aligned pieces of the sorted order return its bits
+    t8 = build(B.OG_WALK_G8)
+    for sub in (clump_a, clump_b, perm[32 * 3:32 * 9].copy(), np.concatenate([perm[32 * 17:m], perm[n - m:n - m + 64]])):
+        a_s, p_s = B.og_shortrange_accel(t8, dev(sub), None)
+        assert B.og_tree_stats(t8)["walk_targets_per_warp"] == 8
+        assert same_bits(a_s, p_s, sub), "sub-list under OG_WALK_G8 differs from the sparse full call"
+    B.og_tree_free(t8)
+    # and the other way round: the sparse list forced to 32 per warp returns the identity call's bits
+    t32 = build(B.OG_WALK_G32)
+    a_f, p_f = B.og_shortrange_accel(t32, dev(full), None)
+    assert B.og_tree_stats(t32)["walk_targets_per_warp"] == 32
+    idx = torch.from_numpy(full.astype(np.int64)).cuda()
+    assert torch.equal(a_f, a_id[idx]) and torch.equal(p_f, p_id[idx])
+    assert B.og_tree_status(t32) == B.OG_OK
+    B.og_tree_free(t32)
+    with pytest.raises(B.OgError):
+        build(B.OG_WALK_G8 | B.OG_WALK_G32)

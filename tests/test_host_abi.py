@@ -73,6 +73,10 @@ def test_argument_errors_and_no_cpu_fallback(B):
         t = B._lib.og_tree_build(buf, buf, buf, 16, C.c_float(1.0), C.byref(p), None)
         assert not t and b"no CUDA device" in B._lib.og_last_error()
     assert B._lib.og_shortrange_accel(None, None, 0, None, None, None, None) == B.OG_ERR_INVALID_ARG
+    # the two grouping flags of the walk exclude each other (og.h)
+    p = B.make_params(0.01, flags=B.OG_PERIODIC | B.OG_WALK_G8 | B.OG_WALK_G32)
+    t = B._lib.og_tree_build(None, None, None, 16, C.c_float(1.0), C.byref(p), None)
+    assert not t and b"OG_WALK_G32" in B._lib.og_last_error()
 
 
 def test_new_rows_reject_bad_arguments_without_a_device(B):
