@@ -258,12 +258,17 @@ int og_shortrange_accel_host(const float *pos, const float *mass, const float *s
  *   active_idx u32 [n_active] original indices of the targets, or NULL -> all n in identity order
  *   (n_active == n); acc_out f32 [n_active][3], pot_out f32 [n_active] or NULL, overwritten.  Enqueues on `stream`.
  *   The mass assignment uses floating-point atomics: results are reproducible to fp32 rounding, not bit for bit.
+ *   An active_idx entry >= n cannot be served: that target gets a zero force and potential, and the mistake is latched
+ *   in the handle (the call itself only enqueues and still returns OG_OK).
+ * og_pm_status: synchronises `stream` and returns OG_OK, or OG_ERR_INVALID_ARG if any og_pm_longrange on this handle met
+ *   an active_idx entry >= n (og_last_error says so); latched until og_pm_free, like og_tree_status for a tree.
  * og_pm_free: synchronises `stream`, releases plans and grids.  NULL is ignored.
  */
 typedef struct og_pm og_pm;
 og_pm *og_pm_create(uint32_t ng, float box, float r_s, float G, og_stream stream);
 int og_pm_longrange(og_pm *pm, const float *pos, const float *mass, uint64_t n, const uint32_t *active_idx,
                     uint64_t n_active, float *acc_out, float *pot_out, og_stream stream);
+int og_pm_status(const og_pm *pm, og_stream stream);
 void og_pm_free(og_pm *pm, og_stream stream);
 
 /* ---- row f2: the time-step shell around the force calls --------------------------------- */
@@ -288,6 +293,10 @@ void og_pm_free(og_pm *pm, og_stream stream);
  *                   by one level only at a tick the larger step divides; vel += acc (dt_old + dt_new) / 2 (first != 0:
  *                   start of the integration, wanted bin taken as is, opening half kick dt_new / 2 only); bin and
  *                   a_old f32 [n] (= |a|, the next walk's opening-criterion input) updated.  Enqueues.
+ *                   status: DEVICE u32 [1] owned (and zeroed) by the caller, or NULL.  An active_idx entry >= n is
+ *                   skipped (no particle is touched for it); with a status word the mistake is also recorded there, the bit
+ *                   OG_TS_BAD_INDEX OR-ed in, for the caller to read when it next synchronises -- a corrupted
+ *                   active list otherwise shows only as particles that stop moving.
  * scratch: DEVICE, og_ts_scratch_bytes(n) bytes.  bmax <= 40.
  */
 size_t og_ts_scratch_bytes(uint64_t n);
@@ -298,7 +307,8 @@ int og_ts_active_list(const uint8_t *bin, uint64_t n, uint64_t tick, uint32_t bm
                       uint64_t *n_active_host, void *scratch, size_t scratch_bytes, og_stream stream);
 int og_ts_kick(float *vel, uint8_t *bin, float *a_old, const uint32_t *active_idx, uint64_t n, uint64_t n_active,
                const float *acc, const float *soft, float eta, float dt_max, uint32_t bmax, uint64_t tick, int first,
-               og_stream stream);
+               uint32_t *status, og_stream stream);
+#define OG_TS_BAD_INDEX 8u   /* og_ts_kick status bit: some active_idx entry was >= n */
 
 /* ---- row f3: SPH density / smoothing length on the same tree -------------------------------- */
 

@@ -137,7 +137,9 @@ def _load():
     lib.og_sph_density.restype = C.c_int
     lib.og_sph_density.argtypes = [vp, u32p, u64, C.c_float, C.c_float, vp, vp, vp, vp, vp]
     lib.og_ts_kick.restype = C.c_int
-    lib.og_ts_kick.argtypes = [vp, vp, vp, u32p, u64, u64, vp, vp, C.c_float, C.c_float, C.c_uint32, u64, C.c_int, vp]
+    lib.og_ts_kick.argtypes = [vp, vp, vp, u32p, u64, u64, vp, vp, C.c_float, C.c_float, C.c_uint32, u64, C.c_int, vp, vp]
+    lib.og_pm_status.restype = C.c_int
+    lib.og_pm_status.argtypes = [vp, vp]
     return lib
 
 
@@ -146,7 +148,7 @@ _lib = _load()
 EXPORTS = ("og_tree_workspace_bytes", "og_tree_build", "og_shortrange_accel", "og_tree_get", "og_tree_status",
            "og_tree_stats", "og_tree_free", "og_last_error", "og_morton_keys", "og_radix_sort_scratch_bytes",
            "og_radix_sort_pairs", "og_radix_sort_pairs_noalloc", "og_shortrange_accel_host", "og_trim", "og_pm_create", "og_pm_longrange",
-           "og_pm_free", "og_ts_scratch_bytes", "og_ts_drift", "og_ts_next_tick", "og_ts_active_list", "og_ts_kick",
+           "og_pm_free", "og_pm_status", "og_ts_scratch_bytes", "og_ts_drift", "og_ts_next_tick", "og_ts_active_list", "og_ts_kick",
            "og_sph_density", "og_shortrange_accel_ext", "og_domain_cell_hist", "og_domain_owner", "og_let_export_list",
            "og_let_accumulate")
 
@@ -389,6 +391,14 @@ def og_pm_longrange(pm: Pm, pos: torch.Tensor, mass: torch.Tensor, active_idx: t
     return acc, pot
 
 
+def og_pm_status(pm: Pm, stream=None) -> int:
+    """Synchronises the stream; OG_OK, or OG_ERR_INVALID_ARG if an og_pm_longrange on this handle met a bad active index."""
+    return int(_lib.og_pm_status(pm.handle, _stream(stream)))
+
+
+OG_TS_BAD_INDEX = 8
+
+
 def og_pm_free(pm: Pm, stream=None):
     if pm.handle:
         h, pm.handle = pm.handle, 0
@@ -424,11 +434,14 @@ def og_ts_active_list(bins: torch.Tensor, tick: int, bmax: int, active_idx: torc
 
 def og_ts_kick(vel: torch.Tensor, bins: torch.Tensor, a_old: torch.Tensor, active_idx: torch.Tensor | None, n_active: int,
                acc: torch.Tensor, soft: torch.Tensor, eta: float, dt_max: float, bmax: int, tick: int, first: bool,
-               stream=None):
+               status: torch.Tensor | None = None, stream=None):
+    """status: int32 CUDA tensor [1] zeroed by the caller (or None): bit OG_TS_BAD_INDEX is set when an active_idx entry
+    is >= n (og.h)."""
     _check(_lib.og_ts_kick(_dev(vel, torch.float32, "vel"), _dev(bins, torch.uint8, "bin"), _dev(a_old, torch.float32, "a_old"),
                            None if active_idx is None else _dev(active_idx, torch.int32, "active_idx"), int(vel.shape[0]),
                            int(n_active), _dev(acc, torch.float32, "acc"), _dev(soft, torch.float32, "soft"), float(eta),
-                           float(dt_max), int(bmax), int(tick), 1 if first else 0, _stream(stream)))
+                           float(dt_max), int(bmax), int(tick), 1 if first else 0, _dev(status, torch.int32, "status"),
+                           _stream(stream)))
 
 
 def og_sph_density(tree: Tree, n_des: float, active_idx: torch.Tensor | None = None, h_guess: torch.Tensor | None = None,

@@ -27,6 +27,7 @@ struct og_pm {
     float4 *fgrid;         // [ng^3] (a_x, a_y, a_z, phi)
     float *k2tab;          // [ng] (2 pi n / L)^2, n in (-ng/2, ng/2]
     float *dctab;          // [ng] 1 / sinc^4(pi n / ng): the CIC window divided out twice, per axis
+    uint32_t *d_status;    // [1] latched OG_DEV_* bits of the calls on this handle (og_pm_status)
     void *arena;
 };
 
@@ -190,7 +191,7 @@ extern "C" og_pm *og_pm_create(uint32_t ng, float box, float r_s, float G, og_st
     pm->ng = ng; pm->box = box; pm->r_s = r_s; pm->G = G; pm->device = dev; pm->have_plans = false; pm->arena = nullptr;
     const size_t n3 = (size_t)ng * ng * ng, nk = (size_t)ng * ng * (ng / 2 + 1);
     const size_t o_m = 0, o_k = o_m + align256(n3 * 4), o_f = o_k + align256(nk * 8), o_t = o_f + align256(n3 * 16),
-                 o_d = o_t + align256(ng * 4), total = o_d + align256(ng * 4);
+                 o_d = o_t + align256(ng * 4), o_s = o_d + align256(ng * 4), total = o_s + 256;
     if (cudaMalloc(&pm->arena, total) != cudaSuccess) {
         (void)cudaGetLastError();
         og_set_error("og_pm_create: cudaMalloc(%zu bytes) failed", total);
@@ -199,7 +200,7 @@ extern "C" og_pm *og_pm_create(uint32_t ng, float box, float r_s, float G, og_st
     }
     char *b = (char *)pm->arena;
     pm->mgrid = (float *)(b + o_m); pm->kgrid = (float2 *)(b + o_k); pm->fgrid = (float4 *)(b + o_f);
-    pm->k2tab = (float *)(b + o_t); pm->dctab = (float *)(b + o_d);
+    pm->k2tab = (float *)(b + o_t); pm->dctab = (float *)(b + o_d); pm->d_status = (uint32_t *)(b + o_s);
     // per-axis tables in fp64 on the host (R32): k^2 and the doubly divided CIC window
     std::vector<float> k2(ng), dc(ng);
     const double PI = 3.14159265358979323846;
@@ -211,7 +212,8 @@ extern "C" og_pm *og_pm_create(uint32_t ng, float box, float r_s, float G, og_st
         const double s = (n == 0) ? 1.0 : sin(a) / a;
         dc[j] = (float)(1.0 / (s * s * s * s));
     }
-    bool ok = cudaMemcpyAsync(pm->k2tab, k2.data(), ng * 4, cudaMemcpyHostToDevice, st) == cudaSuccess &&
+    bool ok = cudaMemsetAsync(pm->d_status, 0, 256, st) == cudaSuccess &&
+              cudaMemcpyAsync(pm->k2tab, k2.data(), ng * 4, cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaMemcpyAsync(pm->dctab, dc.data(), ng * 4, cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaStreamSynchronize(st) == cudaSuccess;      // the host tables go out of scope
     if (ok) {
@@ -261,8 +263,22 @@ extern "C" int og_pm_longrange(og_pm *pm, const float *pos, const float *mass, u
     k_pm_gradient<<<(unsigned)((n3 + 255) / 256), 256, 0, st>>>(pm->mgrid, ng, (4.0f / 3.0f) / (2.0f * delta),
                                                                 (1.0f / 3.0f) / (4.0f * delta), pm->fgrid);
     k_pm_interp<<<(unsigned)((n_active + 255) / 256), 256, 0, st>>>(pos, active_idx, n, n_active, inv_delta, ng, pm->fgrid,
-                                                                   acc_out, pot_out, nullptr);
+                                                                   acc_out, pot_out, pm->d_status);
     OG_CUDA_TRY(cudaGetLastError(), return OG_ERR_CUDA);
+    return OG_OK;
+}
+
+extern "C" int og_pm_status(const og_pm *pm, og_stream stream)
+{
+    og_set_error("%s", "");
+    if (!pm) { og_set_error("og_pm_status: pm is NULL"); return OG_ERR_INVALID_ARG; }
+    uint32_t bits = 0;
+    OG_CUDA_TRY(cudaMemcpyAsync(&bits, pm->d_status, sizeof(bits), cudaMemcpyDeviceToHost, (cudaStream_t)stream), return OG_ERR_CUDA);
+    OG_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream), return OG_ERR_CUDA);
+    if (bits & OG_DEV_BAD_INDEX) {
+        og_set_error("og_pm_longrange: an active_idx entry was >= n (such targets were given a zero force)");
+        return OG_ERR_INVALID_ARG;
+    }
     return OG_OK;
 }
 

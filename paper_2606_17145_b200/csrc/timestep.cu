@@ -174,6 +174,8 @@ k_ts_kick(float *__restrict__ vel, uint8_t *__restrict__ bin, float *__restrict_
     a_old[i] = an;                                                          // R41
 }
 
+static_assert(OG_TS_BAD_INDEX == OG_DEV_BAD_INDEX, "og.h's status bit of og_ts_kick is the bit k_ts_kick sets");
+
 inline size_t ts_tiles(uint64_t n) { return (size_t)((n + TS_TILE - 1) / TS_TILE); }
 
 }  // namespace
@@ -241,7 +243,7 @@ extern "C" int og_ts_active_list(const uint8_t *bin, uint64_t n, uint64_t tick, 
 
 extern "C" int og_ts_kick(float *vel, uint8_t *bin, float *a_old, const uint32_t *active_idx, uint64_t n,
                           uint64_t n_active, const float *acc, const float *soft, float eta, float dt_max, uint32_t bmax,
-                          uint64_t tick, int first, og_stream stream)
+                          uint64_t tick, int first, uint32_t *status, og_stream stream)
 {
     og_set_error("%s", "");
     if (n_active == 0) return OG_OK;
@@ -252,7 +254,7 @@ extern "C" int og_ts_kick(float *vel, uint8_t *bin, float *a_old, const uint32_t
     }
     k_ts_kick<<<(unsigned)((n_active + 255) / 256), 256, 0, (cudaStream_t)stream>>>(vel, bin, a_old, active_idx, n, n_active,
                                                                                    acc, soft, eta, dt_max, bmax, tick, first,
-                                                                                   nullptr);
+                                                                                   status);
     OG_CUDA_TRY(cudaGetLastError(), return OG_ERR_CUDA);
     return OG_OK;
 }

@@ -72,6 +72,23 @@ def test_pm_active_subset_ragged_and_bad_index(B):
     assert a0.shape == (0, 3)
     with pytest.raises(B.OgError):
         B.og_pm_create(33, w.L, r_s)
+    # og.h: an active_idx entry >= n gets a zero force and is latched in the handle (og_pm_status); the other targets
+    # are unaffected
+    assert B.og_pm_status(pm) == B.OG_OK
+    good = torch.from_numpy(act[:64].view(np.int32)).cuda()
+    a_g, p_g = B.og_pm_longrange(pm, pos, mass, good)
+    assert B.og_pm_status(pm) == B.OG_OK
+    bad = good.clone()
+    bad[7] = w.n                                                           # one past the end
+    bad[40] = -1                                                           # 0xffffffff
+    a_b, p_b = B.og_pm_longrange(pm, pos, mass, bad)
+    assert B.og_pm_status(pm) == B.OG_ERR_INVALID_ARG and "active_idx" in B.og_last_error()
+    keep = torch.ones(64, dtype=torch.bool, device="cuda")
+    keep[7] = keep[40] = False
+    assert torch.equal(a_b[keep], a_g[keep]) and torch.equal(p_b[keep], p_g[keep])
+    assert float(a_b[~keep].abs().max()) == 0.0 and float(p_b[~keep].abs().max()) == 0.0
+    B.og_pm_longrange(pm, pos, mass, good)
+    assert B.og_pm_status(pm) == B.OG_ERR_INVALID_ARG                      # latched until the handle is freed
     B.og_pm_free(pm)
 
 

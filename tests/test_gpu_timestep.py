@@ -97,6 +97,41 @@ def test_kick_bins_a_old_exact_and_velocity(B, first):
     assert len(set(new.tolist())) > 4                                          # the test really spans several bins
 
 
+def test_kick_records_a_bad_active_index(B):
+    """og.h (og_ts_kick): an active_idx entry >= n is skipped -- no particle is touched for it -- and, when the caller
+    passes a status word, recorded there as OG_TS_BAD_INDEX; a clean list leaves the word at zero, and the entries next
+    to the bad ones are kicked as usual."""
+    import torch
+    rng = np.random.default_rng(9)
+    n, bmax, eta, dt_max = 4099, 6, 0.025, 0.0625
+    eps = np.full(n, 2e-3, np.float32)
+    vel = rng.standard_normal((n, 3)).astype(np.float32)
+    bins = rng.integers(0, bmax + 1, n).astype(np.uint8)
+    act = rng.choice(n, 600, replace=False).astype(np.uint32)
+    acc = rng.standard_normal((600, 3)).astype(np.float32)
+
+    def run(a, status):
+        dv, db, da = _t(vel), _t(bins), torch.zeros(n, device="cuda")
+        B.og_ts_kick(dv, db, da, _t(a.view(np.int32)), a.shape[0], _t(acc), _t(eps), eta, dt_max, bmax, 0, False, status)
+        torch.cuda.synchronize()
+        return dv.cpu().numpy(), db.cpu().numpy(), da.cpu().numpy()
+
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    v0, b0, a0 = run(act, status)
+    assert int(status[0]) == 0
+    bad = act.copy()
+    bad[[5, 333]] = [n, 0xffffffff]
+    v1, b1, a1 = run(bad, status)
+    assert int(status[0]) == B.OG_TS_BAD_INDEX
+    skipped = act[[5, 333]]
+    same = np.ones(n, bool)
+    same[skipped] = False
+    assert np.array_equal(v1[same], v0[same]) and np.array_equal(b1[same], b0[same]) and np.array_equal(a1[same], a0[same])
+    assert np.array_equal(v1[skipped], vel[skipped]) and np.array_equal(b1[skipped], bins[skipped])   # untouched
+    v2, b2, a2 = run(bad, None)                                   # no status word: same skipping, nothing recorded
+    assert np.array_equal(v2, v1) and np.array_equal(b2, b1)
+
+
 def test_whole_loop_matches_the_oracle_stepper(B):
     """K synchronisation steps of a small clustered box: CUDA walk + og_ts_* against oracle walk + oracle stepper."""
     import torch
