@@ -85,7 +85,9 @@ def test_pm_active_subset_ragged_and_bad_index(B):
     assert B.og_pm_status(pm) == B.OG_ERR_INVALID_ARG and "active_idx" in B.og_last_error()
     keep = torch.ones(64, dtype=torch.bool, device="cuda")
     keep[7] = keep[40] = False
-    assert torch.equal(a_b[keep], a_g[keep]) and torch.equal(p_b[keep], p_g[keep])
+    # (two PM calls agree to fp32 rounding only: the mass assignment sums with atomics, og.h)
+    assert float((a_b[keep] - a_g[keep]).abs().max()) <= 1e-4 * float(a_g.abs().max())
+    assert float((p_b[keep] - p_g[keep]).abs().max()) <= 1e-4 * float(p_g.abs().max())
     assert float(a_b[~keep].abs().max()) == 0.0 and float(p_b[~keep].abs().max()) == 0.0
     B.og_pm_longrange(pm, pos, mass, good)
     assert B.og_pm_status(pm) == B.OG_ERR_INVALID_ARG                      # latched until the handle is freed
