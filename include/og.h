@@ -347,7 +347,10 @@ int og_sph_density(const og_tree *tree, const uint32_t *active_idx, uint64_t n_a
  * domain builds the tree of its own particles in the full box (og_tree_build); the force on a target is the sum of the
  * walks of all domains' trees with the target's own (x, h, a_old): og_shortrange_accel on its home tree (self excluded),
  * og_shortrange_accel_ext on the others, where it is an external point.  A target is exported to a domain only if it is
- * within r_cut of one of that domain's top-cell boxes (a domain farther away contributes exactly nothing).  The ranks
+ * within r_cut of one of that domain's top-cell boxes: the tight boxes of its tree's nodes at level 2 when
+ * r_cut <= 0.05 box, at level 1 otherwise (and of shallower leaves).  A domain farther away then contributes exactly
+ * nothing: nodes at that level and below are culled, and a shallower node that is accepted instead of opened has the
+ * target outside its 0.6 l guard box, at least 0.1 l >= r_cut from its centre of mass (R52).  The ranks
  * exchange particles, boxes, targets and results with NCCL all-to-all / all-gather in the host layer
  * (paper_2606_17145_b200/let.py); the calls below are its device-side steps.  All pointers DEVICE unless named HOST.
  *

@@ -14,8 +14,13 @@ decomposition, Springel 2005):
        (x, h, a_old): its home domain's walk excludes the target itself by slot (primary), the other domains' walks
        treat it as an external point (secondary, oracle.walk_ext).  Summed in the order home, then domains ascending.
   R52  a target is exported to domain q only if it lies within r_cut of the bounding box of one of q's "top cells"
-       (the nodes of q's tree at level 2, or shallower leaves; nearest periodic image, box-to-point distance);
-       a domain farther than that contributes exactly nothing (every node is culled, R17), so the filter is exact.
+       (the nodes of q's tree at level 2 when r_cut <= 0.05 L, else at level 1, or shallower leaves; nearest periodic
+       image, box-to-point distance).  A domain farther than that contributes exactly nothing, so the filter is exact:
+       the nodes at the chosen level and below are culled (R17); a node ABOVE that level which is not opened has the
+       target outside its 0.6 l guard box (R15), i.e. at least 0.1 l away from its cell and hence from its centre of
+       mass -- the root (l = L) is therefore always opened, and a level-1 node (l = L / 2) that is accepted lies
+       >= 0.05 L >= r_cut away and adds nothing (R21: nothing beyond r_cut).  With r_cut > 0.05 L that last step fails
+       (an accepted level-1 node can be within r_cut although none of its level-2 children's boxes is), hence level 1.
   R53  a_old of a target is one number (R23) used in every domain's walk.
 
 Only tests/ may import this module; it calls oracle/ only.
@@ -50,6 +55,11 @@ def owners(keys: np.ndarray, R: int):
     return (np.searchsorted(S, cell, side="right") - 1).astype(np.int32), S
 
 
+def top_level(r_cut: float, L: float) -> int:
+    """R52: the level whose boxes make the export filter exact."""
+    return 2 if r_cut <= 0.05 * L else 1
+
+
 def top_boxes(tree: "oracle.Tree", level: int = 2):
     """R52: tight AABBs (lo, hi) of the tree's nodes at `level`, and of leaves above it."""
     sel = (tree.level == level) | ((tree.level < level) & (tree.n_child == 0))
@@ -68,8 +78,9 @@ def within_reach(x: np.ndarray, lo: np.ndarray, hi: np.ndarray, r_cut: float, L:
     return out
 
 
-def let_walk(pos, mass, eps, params, R: int, active_idx=None, a_old=None, export_all: bool = False):
-    """R49..R53 -> (acc f64[n_t][3], pot f64[n_t], info dict) in active order."""
+def let_walk(pos, mass, eps, params, R: int, active_idx=None, a_old=None, export_all: bool = False, level=None):
+    """R49..R53 -> (acc f64[n_t][3], pot f64[n_t], info dict) in active order.  `level` overrides R52's choice of the
+    top-cell level (tests use it to show that level 2 is not exact for r_cut > 0.05 L)."""
     pos = np.ascontiguousarray(pos, np.float32)
     mass = np.ascontiguousarray(mass, np.float32)
     eps = np.ascontiguousarray(eps, np.float32)
@@ -99,7 +110,7 @@ def let_walk(pos, mass, eps, params, R: int, active_idx=None, a_old=None, export
     for q in range(R):                                   # secondary: domains ascending
         if trees[q] is None:
             continue
-        lo, hi = top_boxes(trees[q])
+        lo, hi = top_boxes(trees[q], top_level(r_cut, L) if level is None else level)
         k = np.flatnonzero(t_own != q)
         if not export_all:
             k = k[within_reach(pos[act[k]], lo, hi, r_cut, L)]

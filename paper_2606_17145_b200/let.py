@@ -193,7 +193,9 @@ def let_forces(B, doms: dict, ex, box: float, prm, geometric: bool = False, want
             continue
         trees[r] = B.og_tree_build(d.pos, d.mass, d.eps, box, prm)
         mark("build")
-        boxes[r] = top_boxes(B, trees[r])
+        # R52: level-2 boxes are an exact filter only while an accepted level-1 node (target >= 0.05 box away from
+        # its cell, outside the guard box) cannot reach inside r_cut; coarser meshes take the level-1 boxes
+        boxes[r] = top_boxes(B, trees[r], 2 if r_cut <= 0.05 * float(box) else 1)
         a_old = None if geometric else d.a_old
         if na:
             acc[r], pot[r] = B.og_shortrange_accel(trees[r], d.active, a_old, want_pot=want_pot)

@@ -93,6 +93,38 @@ def test_export_filter_drops_exactly_nothing_and_really_filters():
         assert i1["n_local"].sum() == w.n and i1["n_local"].min() > 0
 
 
+def test_export_filter_level_follows_r_cut():
+    """R52: level-2 top boxes are exact only for r_cut <= 0.05 L.  Hand-built case with r_cut = 0.18 L: domain 0 is two
+    clumps in different level-2 cells of one level-1 octant; targets of domain 1 sit 6..9 beyond that octant's face
+    (outside its 0.6 l guard box), more than r_cut from either clump's box but 8..11 from the octant's centre of mass.
+    With a large a_old the level-1 node is accepted and adds a non-zero monopole: a level-2 filter drops it, the rule's
+    level-1 filter does not."""
+    rng = np.random.default_rng(11)
+    L, r_s = 100.0, 4.0                                           # r_cut = 18 > 0.05 L
+    clump = lambda c, m: (np.asarray(c) + rng.uniform(-0.5, 0.5, (m, 3))).astype(np.float32)
+    pos = np.concatenate([clump((48.0, 5.0, 25.0), 50), clump((48.0, 45.0, 25.0), 50), clump((57.5, 25.0, 25.0), 100)])
+    n = pos.shape[0]
+    mass = np.full(n, 1.0, np.float32)
+    eps = np.full(n, 0.01, np.float32)
+    prm = oracle.make_params(L, r_s, alpha=0.005, theta=0.5, leaf_max=8)
+    a_old = np.full(n, 1.0e6, np.float32)                         # every node outside its guards is accepted
+    a0, p0, i0 = let.let_walk(pos, mass, eps, prm, 2, a_old=a_old, export_all=True)
+    assert list(i0["n_local"]) == [100, 100]                      # the two clumps of the octant are domain 0
+    assert let.top_level(18.0, L) == 1 and let.top_level(5.0, L) == 2 and let.top_level(5.0001, L) == 1
+    a1, p1, i1 = let.let_walk(pos, mass, eps, prm, 2, a_old=a_old)
+    assert np.array_equal(a0, a1) and np.array_equal(p0, p1)      # the rule's filter is exact
+    a2, p2, i2 = let.let_walk(pos, mass, eps, prm, 2, a_old=a_old, level=2)
+    lost = np.abs(a0 - a2).sum(1) > 0
+    assert lost[100:].any() and not lost[:100].any()              # level 2 loses the monopole for targets of domain 1
+    assert i2["n_exported"].sum() < i1["n_exported"].sum() <= i0["n_exported"].sum()
+    # the small-r_cut side of the rule on a random box: level 2 chosen, exact, and a real filter
+    w, prm_s = _small(20, 5, r_s=1.0)                             # r_cut = 4.5 <= 0.05 L
+    ao = (rng.random(w.n) * 0.01 + 1e-4).astype(np.float32)
+    b0, q0, j0 = let.let_walk(w.pos, w.mass, w.eps, prm_s, 3, a_old=ao, export_all=True)
+    b1, q1, j1 = let.let_walk(w.pos, w.mass, w.eps, prm_s, 3, a_old=ao)
+    assert np.array_equal(b0, b1) and np.array_equal(q0, q1) and j1["n_exported"].sum() < j0["n_exported"].sum()
+
+
 def test_domain_decomposed_tree_force_converges_to_the_global_direct_sum():
     w, prm = _small()
     a_ref, p_ref = oracle.direct(w.pos, w.mass, w.eps, prm)
