@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/og.h: argument checks, device arena layout, stream-ordered
 // launch sequences.  Every step of the path runs in the kernels of this directory; there is no
 // CPU fallback.
+#include <atomic>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -108,6 +109,30 @@ int device_sm_count(int *device_out)
     if (device_out) *device_out = dev;
     return sms;
 }
+
+}  // namespace
+
+// SMs of the current device, for the grid-stride kernels that size their grid as a multiple of it (the sort's histogram
+// pass, the time-step reductions): asked once per device, 148 (a B200) when no device is visible.
+int ogk_sm_count(void)
+{
+    static std::atomic<int> cache[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return 148; }
+    if (dev >= 0 && dev < 64) {
+        const int c = cache[dev].load(std::memory_order_relaxed);
+        if (c > 0) return c;
+    }
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+        (void)cudaGetLastError();
+        return 148;
+    }
+    if (dev >= 0 && dev < 64) cache[dev].store(sms, std::memory_order_relaxed);
+    return sms;
+}
+
+namespace {
 
 // Stream-ordered allocations come from a pool owned by the library whose release threshold is
 // unlimited: a tree arena (GBs) freed by og_tree_free is reused by the next og_tree_build instead

@@ -104,6 +104,9 @@ void og_set_error(const char *fmt, ...);
         }                                                                                \
     } while (0)
 
+// SMs of the current device (cached per device; 148 when none is visible): grid-stride kernels size their grids by it
+int ogk_sm_count(void);
+
 // ---- kernel launchers (one per row of SURVEY.md Sec. 8(a)) ----
 // a1
 cudaError_t ogk_keys(const float *pos, uint64_t n, float box, uint64_t *keys, uint32_t *idx,

@@ -27,6 +27,7 @@ struct og_pm {
     float4 *fgrid;         // [ng^3] (a_x, a_y, a_z, phi)
     float *k2tab;          // [ng] (2 pi n / L)^2, n in (-ng/2, ng/2]
     float *dctab;          // [ng] 1 / sinc^4(pi n / ng): the CIC window divided out twice, per axis
+    size_t arena_bytes;    // grids + tables + the cuFFT work area shared by the two plans
     uint32_t *d_status;    // [1] latched OG_DEV_* bits of the calls on this handle (og_pm_status)
     void *arena;
 };
@@ -190,11 +191,36 @@ extern "C" og_pm *og_pm_create(uint32_t ng, float box, float r_s, float G, og_st
     if (!pm) { og_set_error("host allocation failed"); return nullptr; }
     pm->ng = ng; pm->box = box; pm->r_s = r_s; pm->G = G; pm->device = dev; pm->have_plans = false; pm->arena = nullptr;
     const size_t n3 = (size_t)ng * ng * ng, nk = (size_t)ng * ng * (ng / 2 + 1);
+    // The two plans are made first, without cuFFT's own work areas: the forward and the inverse transform of a call
+    // run one after the other on one stream, so ONE work area of the larger size serves both and sits in the arena.
+    size_t ws_f = 0, ws_b = 0;
+    bool planned = cufftCreate(&pm->plan_r2c) == CUFFT_SUCCESS;
+    if (planned) {
+        planned = cufftCreate(&pm->plan_c2r) == CUFFT_SUCCESS;
+        if (!planned) cufftDestroy(pm->plan_r2c);
+    }
+    if (planned) {
+        planned = cufftSetAutoAllocation(pm->plan_r2c, 0) == CUFFT_SUCCESS && cufftSetAutoAllocation(pm->plan_c2r, 0) == CUFFT_SUCCESS &&
+                  cufftMakePlan3d(pm->plan_r2c, (int)ng, (int)ng, (int)ng, CUFFT_R2C, &ws_f) == CUFFT_SUCCESS &&
+                  cufftMakePlan3d(pm->plan_c2r, (int)ng, (int)ng, (int)ng, CUFFT_C2R, &ws_b) == CUFFT_SUCCESS;
+        if (!planned) { cufftDestroy(pm->plan_r2c); cufftDestroy(pm->plan_c2r); }
+    }
+    if (!planned) {
+        (void)cudaGetLastError();
+        og_set_error("og_pm_create: cuFFT plan creation failed for ng = %u", ng);
+        delete pm;
+        return nullptr;
+    }
+    pm->have_plans = true;
+    const size_t work = ws_f > ws_b ? ws_f : ws_b;
     const size_t o_m = 0, o_k = o_m + align256(n3 * 4), o_f = o_k + align256(nk * 8), o_t = o_f + align256(n3 * 16),
-                 o_d = o_t + align256(ng * 4), o_s = o_d + align256(ng * 4), total = o_s + 256;
+                 o_d = o_t + align256(ng * 4), o_s = o_d + align256(ng * 4), o_w = o_s + 256, total = o_w + align256(work);
+    pm->arena_bytes = total;
     if (cudaMalloc(&pm->arena, total) != cudaSuccess) {
         (void)cudaGetLastError();
-        og_set_error("og_pm_create: cudaMalloc(%zu bytes) failed", total);
+        og_set_error("og_pm_create: cudaMalloc(%zu bytes) failed (ng = %u: %zu bytes of grids + %zu bytes of cuFFT work area)",
+                     total, ng, total - align256(work), work);
+        cufftDestroy(pm->plan_r2c); cufftDestroy(pm->plan_c2r);
         delete pm;
         return nullptr;
     }
@@ -216,17 +242,12 @@ extern "C" og_pm *og_pm_create(uint32_t ng, float box, float r_s, float G, og_st
               cudaMemcpyAsync(pm->k2tab, k2.data(), ng * 4, cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaMemcpyAsync(pm->dctab, dc.data(), ng * 4, cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaStreamSynchronize(st) == cudaSuccess;      // the host tables go out of scope
-    if (ok) {
-        ok = cufftPlan3d(&pm->plan_r2c, (int)ng, (int)ng, (int)ng, CUFFT_R2C) == CUFFT_SUCCESS;
-        if (ok) {
-            ok = cufftPlan3d(&pm->plan_c2r, (int)ng, (int)ng, (int)ng, CUFFT_C2R) == CUFFT_SUCCESS;
-            if (!ok) cufftDestroy(pm->plan_r2c);
-        }
-        pm->have_plans = ok;
-    }
+    if (ok && work)
+        ok = cufftSetWorkArea(pm->plan_r2c, b + o_w) == CUFFT_SUCCESS && cufftSetWorkArea(pm->plan_c2r, b + o_w) == CUFFT_SUCCESS;
     if (!ok) {
         (void)cudaGetLastError();
-        og_set_error("og_pm_create: table upload or cuFFT plan creation failed");
+        og_set_error("og_pm_create: table upload or cuFFT work-area set-up failed");
+        cufftDestroy(pm->plan_r2c); cufftDestroy(pm->plan_c2r);
         cudaFree(pm->arena);
         delete pm;
         return nullptr;

@@ -434,7 +434,8 @@ cudaError_t ogk_radix_sort(uint64_t *keys, uint32_t *vals, uint64_t *keys_alt, u
         e = cudaMemsetAsync(scratch, 0, ((size_t)SORT_MAX_PASSES * 256 + 64 + (size_t)passes * n_tiles * 256) * sizeof(uint32_t), st);
         if (e != cudaSuccess) return e;
         const uint64_t hwant = (n + SORT_THREADS * 16 - 1) / (SORT_THREADS * 16);
-        const unsigned hgrid = (unsigned)(hwant < 148 * 8 ? hwant : 148 * 8);
+        const uint64_t hmax = (uint64_t)ogk_sm_count() * 8;          // 8 resident blocks of 256 threads per SM
+        const unsigned hgrid = (unsigned)(hwant < hmax ? hwant : hmax);
         k_sort_ghist<<<hgrid, SORT_THREADS, 0, st>>>(kin, n, begin_bit, end_bit, passes, ghist);
         k_sort_gscan<<<passes, 256, 0, st>>>(ghist);
         for (int p = 0; p < passes; ++p) {

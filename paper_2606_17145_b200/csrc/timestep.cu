@@ -207,7 +207,8 @@ extern "C" int og_ts_next_tick(const uint8_t *bin, uint64_t n, uint64_t tick, ui
     uint32_t *d_max = reinterpret_cast<uint32_t *>(scratch);
     OG_CUDA_TRY(cudaMemsetAsync(d_max, 0, sizeof(uint32_t), st), return OG_ERR_CUDA);
     const uint64_t want_blocks = (n + 255) / 256;
-    const unsigned grid = (unsigned)(want_blocks < 148 * 16 ? want_blocks : 148 * 16);
+    const uint64_t max_blocks = (uint64_t)ogk_sm_count() * 16;
+    const unsigned grid = (unsigned)(want_blocks < max_blocks ? want_blocks : max_blocks);
     k_ts_maxbin<<<grid, 256, 0, st>>>(bin, n, d_max);
     uint32_t mb = 0;
     OG_CUDA_TRY(cudaMemcpyAsync(&mb, d_max, sizeof(mb), cudaMemcpyDeviceToHost, st), return OG_ERR_CUDA);
