@@ -279,6 +279,7 @@ def run_ours(args):
     w = make_workload(args.workload, 0 if strong else rank)   # strong: every rank holds the same box (and tree)
     n, na = w.n, w.n_active
     prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8)
+    prm.flags |= {"auto": 0, "32": B.OG_WALK_G32, "8": B.OG_WALK_G8}[args.walk_grouping]
     h_pos = torch.from_numpy(w.pos).pin_memory()
     h_mass = torch.from_numpy(w.mass).pin_memory()
     h_eps = torch.from_numpy(w.eps).pin_memory()
@@ -633,6 +634,7 @@ def run_let(args):
         R = max(1, args.let_domains)
         ex, mine = let.LocalExchange(R), list(range(R))
     prm = B.make_params(w.r_s, G=w.G, rcut_over_rs=w.rcut_over_rs, alpha=w.alpha, theta=w.theta, leaf_max=8)
+    prm.flags |= {"auto": 0, "32": B.OG_WALK_G32, "8": B.OG_WALK_G8}[args.walk_grouping]
     active = np.zeros(w.n, bool)
     active[np.arange(w.n) if w.active_idx is None else w.active_idx] = True
 
@@ -686,7 +688,7 @@ def run_let(args):
                 "unit": "particles/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
                 "higher_is_better": True, "scaling": "strong", "dtype": "f32", "data": "synthetic",
                 "config": {"workload": w.name, "n": w.n, "n_active": int(active.sum()), "domains": R,
-                           "exchange": "nccl all-to-all, one process per GPU" if world > 1 else
+                           "walk_grouping": args.walk_grouping, "exchange": "nccl all-to-all, one process per GPU" if world > 1 else
                            f"{R} domains one after the other on one GPU (time = sum over the domains)"},
                 "particles_per_domain": n_loc if world > 1 else [int(d[r].pos.shape[0]) for r in mine],
                 "ms_each_step_rank0": per_step, "ms_median_step_rank0": sorted(per_step)[len(per_step) // 2], "exported_target_copies": int(sum(n_exp)), "checksum_sum_abs_acc_milli": int(sum(chk))}
@@ -769,6 +771,9 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1 << 17)
     ap.add_argument("--ref-sample", type=int, default=1 << 15)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--walk-grouping", default="auto", choices=["auto", "32", "8"],
+                    help="targets per warp of walks with an active list or external targets: chosen by the library (auto) "
+                         "or fixed with OG_WALK_G32 / OG_WALK_G8 (standard step and --scaling let)")
     ap.add_argument("--let-domains", type=int, default=4, help="--scaling let with one process: number of domains emulated")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong", "let"],
                     help="weak (default): one independent box per GPU; strong: one box, every rank builds the tree and walks "

@@ -361,7 +361,10 @@ int og_sph_density(const og_tree *tree, const uint32_t *active_idx, uint64_t n_a
  * og_shortrange_accel_ext  walk of `tree` for n_t targets that are NOT particles of the tree: tpos f32 [n_t][3] in
  *     [0, box), tsoft f32 [n_t] (eps; h = 2.8 eps as in the tree), a_old f32 [n_t] or NULL (geometric criterion);
  *     acc_out f32 [n_t][3], pot_out f32 [n_t] or NULL, overwritten, in the caller's order.  Nothing is excluded.  The
- *     targets are walked in their own Morton order, 32 per warp.  Enqueues; stream rules as og_shortrange_accel.
+ *     targets are walked in their own Morton order, 32 per warp, or 8 per warp when they are sparse against this tree:
+ *     fewer than 1 / 16 of the tree's particles whose keys lie between the first and the last target's key (decided on
+ *     the device; OG_WALK_G32 / OG_WALK_G8 fix it; og_stats.walk_targets_per_warp reports it).  Enqueues; stream rules
+ *     as og_shortrange_accel.
  * og_domain_cell_hist      hist u32 [32768] = particles per level-5 cell of pos f32 [n][3] (overwritten).  Enqueues.
  * og_domain_owner          owner u32 [n] = the d with splitters[d] <= cell < splitters[d + 1]; splitters u32
  *     [n_domains + 1], ascending, splitters[0] = 0, splitters[n_domains] = 32768.  Enqueues.

@@ -427,10 +427,13 @@ extern "C" int og_shortrange_accel_ext(const og_tree *t, const float *tpos, cons
     OG_EXT_TRY(ogk_radix_sort(k0, v0, k1, v1, n_t, 0, 64, tmp + o_sc, &in_alt, st));
     const uint32_t *order = in_alt ? v1 : v0;
     OG_EXT_TRY(ogk_ext_gather(tpos, tsoft, order, n_t, ext, st));
-    OG_EXT_TRY(ogk_walk(t, nullptr, order, n_t, a_old, acc_out, pot_out, st, ext));
+    // grouping as for an active list (og.h), the targets' density taken against the tree's particles in their key range
+    const uint32_t sparse_div = (t->prm.flags & OG_WALK_G8) ? 0u : (t->prm.flags & OG_WALK_G32) ? 0xffffffffu : OG_SPARSE_DIV;
+    OG_EXT_TRY(ogk_ext_sparse(in_alt ? k1 : k0, n_t, t->keys, t->n, sparse_div, t->d_status + 2, st));
+    OG_EXT_TRY(ogk_walk(t, nullptr, order, n_t, a_old, acc_out, pot_out, st, ext, t->d_status + 2));
     OG_EXT_TRY(cudaEventRecord(t->ev_walked, st));
     t->walked = true;
-    t->walk_kind = 1;
+    t->walk_kind = 2;
     OG_EXT_TRY(cudaFreeAsync(tmp, st));
 #undef OG_EXT_TRY
     return OG_OK;

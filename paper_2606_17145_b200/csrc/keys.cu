@@ -146,6 +146,29 @@ k_unpack_slots(const uint64_t *__restrict__ keys, uint64_t n_active, uint32_t *_
     }
 }
 
+// The same decision for targets that are not particles of the tree (og_shortrange_accel_ext): their density is
+// measured against the tree they walk -- `*sparse` = 1 if the n_t targets are fewer than 1 / sparse_div of the tree's
+// particles whose keys lie between the first and the last target key (two binary searches over the tree's sorted keys).
+__global__ void k_ext_sparse(const uint64_t *__restrict__ tkeys, uint64_t n_t, const uint64_t *__restrict__ keys, uint64_t n,
+                             uint32_t sparse_div, uint32_t *__restrict__ sparse)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const uint64_t k_first = tkeys[0], k_last = tkeys[n_t - 1];
+    uint64_t lo = 0, hi = n;                       // first tree slot with key >= k_first
+    while (lo < hi) { const uint64_t m = (lo + hi) >> 1; if (keys[m] < k_first) lo = m + 1; else hi = m; }
+    const uint64_t first = lo;
+    lo = first; hi = n;                            // first tree slot with key > k_last
+    while (lo < hi) { const uint64_t m = (lo + hi) >> 1; if (keys[m] <= k_last) lo = m + 1; else hi = m; }
+    *sparse = (sparse_div == 0u || n_t * (uint64_t)sparse_div < lo - first) ? 1u : 0u;   // 0: forced (OG_WALK_G8)
+}
+
+cudaError_t ogk_ext_sparse(const uint64_t *tkeys_sorted, uint64_t n_t, const uint64_t *tree_keys, uint64_t n, uint32_t sparse_div,
+                           uint32_t *sparse, cudaStream_t st)
+{
+    k_ext_sparse<<<1, 32, 0, st>>>(tkeys_sorted, n_t, tree_keys, n, sparse_div, sparse);
+    return cudaGetLastError();
+}
+
 cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_perm, uint64_t n,
                              uint64_t n_active, uint64_t *keys, uint32_t *vals, uint32_t *d_status,
                              cudaStream_t st)

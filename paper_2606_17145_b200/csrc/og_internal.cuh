@@ -131,7 +131,7 @@ cudaError_t ogk_cover(const og_tree *t, cudaStream_t st);
 // a6 + a7
 cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out,
                      uint64_t n_active, const float *a_old, float *acc_out, float *pot_out,
-                     cudaStream_t st, const float4 *ext = nullptr);
+                     cudaStream_t st, const float4 *ext = nullptr, const uint32_t *ext_sparse = nullptr);
 size_t ogk_walk_spill_bytes(int sm_count, uint32_t spill_entries);
 uint32_t ogk_walk_spill_entries(const og_params *p);
 // f3
@@ -155,4 +155,6 @@ cudaError_t ogk_active_slots(const uint32_t *active_idx, const uint32_t *inv_per
                              cudaStream_t st);
 cudaError_t ogk_unpack_slots(const uint64_t *keys, uint64_t n_active, uint32_t *slots, uint32_t sparse_div,
                              uint32_t *sparse, cudaStream_t st);
+cudaError_t ogk_ext_sparse(const uint64_t *tkeys_sorted, uint64_t n_t, const uint64_t *tree_keys, uint64_t n, uint32_t sparse_div,
+                           uint32_t *sparse, cudaStream_t st);
 #define OG_SPARSE_DIV 16u  // an active list that fills fewer than 1 / 16 of its Morton range counts as sparse (8 targets per warp)

@@ -993,11 +993,10 @@ cudaError_t launch_g(const og_tree *t, WalkArgs a, cudaStream_t st)
 template <bool GEOM, bool POT, bool COUNT>
 cudaError_t launch(const og_tree *t, WalkArgs &a, cudaStream_t st)
 {
-    if (a.tgt_slot == nullptr) {
-        a.sel_flag = nullptr; a.sel = 0u;
+    if (a.sel_flag == nullptr) {       // identity list: always dense
+        a.sel = 0u;
         return launch_g<GEOM, POT, COUNT, 32>(t, a, st);
     }
-    a.sel_flag = t->d_status + 2;
     a.sel = 0u;
     cudaError_t e = launch_g<GEOM, POT, COUNT, 32>(t, a, st);
     if (e != cudaSuccess) return e;
@@ -1018,10 +1017,14 @@ size_t ogk_walk_spill_bytes(int sm_count, uint32_t spill_entries)
 }
 
 cudaError_t ogk_walk(const og_tree *t, const uint32_t *tgt_slot, const uint32_t *tgt_out, uint64_t n_active,
-                     const float *a_old, float *acc_out, float *pot_out, cudaStream_t st, const float4 *ext)
+                     const float *a_old, float *acc_out, float *pot_out, cudaStream_t st, const float4 *ext,
+                     const uint32_t *ext_sparse)
 {
     WalkArgs a;
     a.ext = ext;
+    // the device flag that picks 32 or 8 targets per warp: written by k_unpack_slots for an explicit active list, by
+    // k_ext_sparse for external targets (the caller passes where); none for the identity list
+    a.sel_flag = tgt_slot ? t->d_status + 2 : ext_sparse;
     a.com = t->node_com; a.cell = t->node_cell; a.lo = t->node_lo; a.hi = t->node_hi;
     a.info = t->node_info; a.rec = t->node_rec; a.spos = t->spos; a.sh = t->sh;
     a.tgt_slot = tgt_slot; a.tgt_out = tgt_out; a.a_old = a_old; a.acc_out = acc_out; a.pot_out = pot_out;

@@ -215,3 +215,28 @@ def test_external_targets_on_top_of_tree_particles_and_across_the_wall(B):
     check_acc(a2.cpu().numpy()[nz], ao2[nz], what="ext on a counting tree")
     assert B.og_tree_status(tc) == B.OG_OK and float(guard.min()) == 7.0
     B.og_tree_free(tc)
+
+
+def test_external_targets_grouping_follows_their_density_against_the_tree(B):
+    """og.h (og_shortrange_accel_ext): external targets are walked 8 per warp when they are fewer than 1 / 16 of the
+    tree's particles in the key range they span, else 32 per warp; OG_WALK_G32 / OG_WALK_G8 fix it and
+    og_stats.walk_targets_per_warp reports it.  Either grouping meets the oracle within the walk's gates."""
+    import torch
+    w = W.make("nfw256", small=True)
+    rng = np.random.default_rng(23)
+    pos, mass, eps = to_dev(w)
+    ot = oracle.build_tree(w.pos, w.mass, w.eps, oracle_params(w))
+    few = (rng.random((300, 3)) * w.L).astype(np.float32)                    # 300 x 16 << n: sparse
+    many = np.mod(w.pos[rng.choice(w.n, 20000, replace=False)].astype(np.float64) + 0.01, w.L).astype(np.float32)   # dense
+    many[many >= w.L] = 0.0
+    for tpos, expect in ((few, 8), (many, 32)):
+        teps = np.full(tpos.shape[0], float(w.eps[0]), np.float32)
+        ao, po, _ = oracle.walk_ext(ot, tpos, oracle.particle_h(teps), None)
+        tp_d, te_d = torch.from_numpy(tpos).cuda(), torch.from_numpy(teps).cuda()
+        for flags, tpw in ((0, expect), (B.OG_WALK_G32, 32), (B.OG_WALK_G8, 8)):
+            tree = B.og_tree_build(pos, mass, eps, w.L, gpu_params(w, flags=flags))
+            a, p = B.og_shortrange_accel_ext(tree, tp_d, te_d, None)
+            assert B.og_tree_stats(tree)["walk_targets_per_warp"] == tpw, (tpos.shape[0], flags)
+            check_acc(a.cpu().numpy(), ao, what=f"ext {tpos.shape[0]} targets, {tpw} per warp")
+            assert B.og_tree_status(tree) == B.OG_OK, B.og_last_error()
+            B.og_tree_free(tree)
