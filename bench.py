@@ -255,7 +255,11 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_full, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "n": w.n, "n_active": w.n_active},
+            # the keys of the repo arm's `config` (same workload, same canonical tree), so that the two lines compare
+            "config": {"workload": w.name, "n": w.n, "n_active": w.n_active, "box": w.L, "r_s": w.r_s, "alpha": w.alpha,
+                       "leaf_max": 8, "n_nodes": int(t.level.shape[0]), "max_level": int(t.level.max()),
+                       "l2_policy": "inputs larger than L2 (no flush): particles + tree > 1.5 GB vs 126 MB L2",
+                       "parallelism": f"oracle on {oracle.num_threads()} host cores (no GPU)"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                              "sample": sample},
             # ms_per_step is not a measured wall time: walk of `sample_targets` targets scaled to all active ones
